@@ -1,0 +1,49 @@
+"""Seeded synthetic workloads shared by the CUDA path's tests/bench and the oracle's tests.
+
+Holds NO arithmetic of the method: only the table of configurations from BASELINE.json
+(`configs`) — process string, sqrt(s), event count, Philox seed, final-state
+masses — and a reader for the text fixtures in tests/golden/.  Momenta themselves are produced
+by each side's own Philox+RAMBO (compared separately), or by the CUDA path and handed to the
+oracle as plain doubles for |M|^2 parity (SURVEY §8c "parity protocol").
+"""
+import os
+
+MT = 173.0
+
+# name -> configuration.  `index` is the position in BASELINE.json `configs`.
+CONFIGS = {
+    "eemumu": dict(index=0, proc="e+ e- > mu+ mu-", sqrt_s=500.0, nevt=16384, seed=1,
+                   masses_final=[0.0, 0.0], precisions=("fp64",)),
+    "ggtt": dict(index=1, proc="g g > t t~", sqrt_s=1500.0, nevt=524288, seed=2,
+                 masses_final=[MT, MT], precisions=("fp64",)),
+    "ggttg": dict(index=2, proc="g g > t t~ g", sqrt_s=1500.0, nevt=524288, seed=3,
+                  masses_final=[MT, MT, 0.0], precisions=("fp64", "fp32")),
+    "ggttgg": dict(index=3, proc="g g > t t~ g g", sqrt_s=1500.0, nevt=524288, seed=4,
+                   masses_final=[MT, MT, 0.0, 0.0], precisions=("fp64", "fp32")),
+    "ggttggg": dict(index=4, proc="g g > t t~ g g g", sqrt_s=1500.0, nevt=262144, seed=5,
+                    masses_final=[MT, MT, 0.0, 0.0, 0.0], precisions=("fp64",)),
+}
+PROC_TO_NAME = {v["proc"]: k for k, v in CONFIGS.items()}
+
+GOLDEN_DIR = os.path.join(os.path.dirname(os.path.abspath(__file__)), "tests", "golden")
+
+
+def read_points(filename):
+    """Parse a tests/golden/*.txt fixture: blocks of
+         point <name> <proc...> | value <float>
+         <E> <px> <py> <pz>     (one line per particle, process order)
+       '#' starts a comment.  Returns list of dict(name, proc, value, momenta)."""
+    pts, cur = [], None
+    with open(os.path.join(GOLDEN_DIR, filename)) as fh:
+        for line in fh:
+            line = line.split("#", 1)[0].strip()
+            if not line:
+                continue
+            if line.startswith("point"):
+                head, val = line.split("|")
+                toks = head.split()
+                cur = dict(name=toks[1], proc=" ".join(toks[2:]), value=float(val.split()[1]), momenta=[])
+                pts.append(cur)
+            else:
+                cur["momenta"].append([float(x) for x in line.split()])
+    return pts
