@@ -1,0 +1,44 @@
+// mg_kernel.cuh — pieces shared by every generated process kernel (not by the oracle).
+//   * the AoSoA momentum layout of the C ABI (include/mg5b200.h):
+//       mom[page][ipar][ievt_in_page][4] doubles, NEPP = 32 events per page, (E,px,py,pz);
+//     a thread's 4-vector is 32 contiguous bytes (two 128-bit loads), a warp reads 1 KiB contiguous.
+//   * helicity index convention: bit (npar-1-i) of h set <=> particle i has lambda = +1.
+//   * mg_procdesc_t: what a generated translation unit registers with the C-ABI layer.
+#pragma once
+#ifdef __CUDACC__
+#include <cuda_runtime.h>
+#endif
+#include <math.h>
+#include "mg_wave.cuh"
+
+constexpr int MG_NEPP = 32;
+
+template <class T, int NPAR>
+MG_DEV void load_momentum(const double* __restrict__ mom, long long ievt, int ipar, mgw::P4<T>& p) {
+  const long long page = ievt / MG_NEPP;
+  const int lane = (int)(ievt % MG_NEPP);
+  const double* src = mom + ((page * NPAR + ipar) * MG_NEPP + lane) * 4;
+#ifdef __CUDA_ARCH__
+  const double2* q = reinterpret_cast<const double2*>(src);
+  const double2 a = __ldg(q), b = __ldg(q + 1);
+  p.c[0] = T(a.x); p.c[1] = T(a.y); p.c[2] = T(b.x); p.c[3] = T(b.y);
+#else
+  p.c[0] = T(src[0]); p.c[1] = T(src[1]); p.c[2] = T(src[2]); p.c[3] = T(src[3]);
+#endif
+}
+
+template <int NPAR> MG_DEV int hel_of(int h, int ipar) {
+  return ((h >> (NPAR - 1 - ipar)) & 1) ? 1 : -1;
+}
+
+#ifdef __CUDACC__
+typedef void (*mg_launch_fn)(int prec, const double* mom, void* me_out, long long nevt, const int* hel_list,
+                             int nhel_run, void* perhel_out, const double* par, cudaStream_t st);
+struct mg_procdesc_t {
+  const char* proc;          // canonical process string
+  int npar, ngluons, ndiagrams, nhel, ncol, denominator;
+  long long flops_per_helicity;   // generator's static count (DFMA = 2)
+  int massive[8];            // 1 where the particle has mass mt
+  mg_launch_fn launch;
+};
+#endif  // __CUDACC__
