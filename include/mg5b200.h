@@ -1,0 +1,129 @@
+/* mg5b200.h — C ABI of the B200-native matrix-element library (libmg5b200.so).
+ *
+ * The hot path of arXiv:2312.02898 ("Madgraph5_aMC@NLO on GPUs and vector CPUs"), standalone-program shape
+ * (Fig. 1b): a batch of random numbers -> RAMBO phase-space points -> per-event
+ * tree-level |M|^2 summed over helicities and colours, evaluated event-parallel on the GPU (PAPER.md:13,
+ * :41, :45).  The caller owns batches; the library is a pure function momenta -> |M|^2 (the shape of the
+ * Fortran<->CUDA bridge of PAPER.md:67-:89, Fig. 1c).  Processes: the set validated in PAPER.md:139 —
+ *     "e+ e- > mu+ mu-", "g g > t t~", "g g > t t~ g", "g g > t t~ g g", "g g > t t~ g g g"
+ * (leading order, fixed couplings: PAPER.md:141).
+ *
+ * Plain C: opaque handle, plain pointers and sizes.  Every `*_dev` pointer is DEVICE memory owned by the
+ * caller (the library never frees or reallocates it); `stream` is a cudaStream_t passed as void* (NULL =
+ * default stream).  All calls return mg_status_t (0 = OK); none throws, exits or prints.  There is no CPU
+ * fallback: without a CUDA device mg_process_create returns MG_ERR_NO_DEVICE.
+ *
+ * Momenta layout (fixed by this ABI; element type double for both precisions): AoSoA pages of
+ * MG_NEPP = 32 events,
+ *       mom[page][ipar][ievt_in_page][4],   4-vector order (E, px, py, pz), GeV, metric (+,-,-,-),
+ * particles in the order of the process string (initial state first).  nevt need not be a multiple of 32
+ * but the buffer must be mg_momenta_bytes(p, nevt) long (whole pages) and 16-byte aligned.
+ * Output: me_out[nevt], double (MG_FP64) or float (MG_FP32): spin- and colour-averaged |M|^2 including the
+ * 1/k! for k identical final-state gluons (denominators 4, 256, 256, 512, 1536), in GeV^(-2(npar-4)).
+ */
+#ifndef MG5B200_H
+#define MG5B200_H
+#include <stddef.h>
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define MG_NEPP 32
+
+typedef struct mg_process mg_process_t; /* opaque, library-owned */
+
+typedef enum {
+  MG_OK = 0,
+  MG_ERR_NULL = -1,       /* a required pointer argument is NULL                       */
+  MG_ERR_BAD_PROC = -2,   /* process string not one of the five generated processes    */
+  MG_ERR_BAD_PARAM = -3,  /* struct_size mismatch, unknown precision / helicity mode   */
+  MG_ERR_BAD_NEVT = -4,   /* nevt < 0                                                  */
+  MG_ERR_ALIGN = -5,      /* a device pointer is not 16-byte aligned                   */
+  MG_ERR_KINEMATICS = -6, /* sqrt_s <= sum of final-state masses                       */
+  MG_ERR_CUDA = -7,       /* a CUDA call failed; text in mg_last_error()               */
+  MG_ERR_NO_DEVICE = -8   /* no CUDA device / bad ordinal                              */
+} mg_status_t;
+
+typedef enum { MG_FP64 = 0, MG_FP32 = 1 } mg_precision_t;
+typedef enum {
+  MG_HEL_FILTER = 0, /* find the non-vanishing helicities on a probe batch (first mg_sigma call) */
+  MG_HEL_ALL = 1     /* always sum all 2^npar helicities                                        */
+} mg_helmode_t;
+
+typedef struct {          /* caller-owned, copied by mg_process_create                              */
+  uint32_t struct_size;   /* = sizeof(mg_params_t)                                                  */
+  int32_t precision;      /* mg_precision_t of the matrix-element kernels (RAMBO is always fp64)    */
+  int32_t helicity_mode;  /* mg_helmode_t                                                           */
+  int32_t device;         /* CUDA ordinal                                                           */
+  double alpha_s;         /* 0.118, fixed                                            */
+  double alpha_ew_inv;    /* 132.507                                                                */
+  double gf;              /* 1.16639e-5 GeV^-2; only used to derive sw2 when sw2 <= 0               */
+  double sw2;             /* > 0 overrides the derived sin^2(theta_W)                               */
+  double mz, gamma_z;     /* 91.188, 2.4414                                                         */
+  double mt, gamma_t;     /* 173.0; gamma_t must be 0 (external on-shell tops; reading A2)*/
+} mg_params_t;
+
+typedef struct {
+  int32_t npar, nfinal, ndiagrams, nhel, ngoodhel, ncolor, denominator, nepp;
+  int64_t flops_per_event_allhel;  /* generator's static FLOP count (FMA = 2), all helicities       */
+  int64_t flops_per_event_goodhel; /* same for the current good-helicity list                       */
+  double masses[8];                /* per particle, process order                                   */
+} mg_info_t;
+
+/* Fills *params with the defaults of BASELINE.json's configs (fp64, helicity filter, device 0). */
+int mg_params_default(mg_params_t* params);
+
+/* Creates the process object: parses `proc` (MG5 syntax, whitespace-insensitive), copies `params`,
+ * selects the generated kernel set, uploads constants.  PAPER.md:45 (per-process generated code). */
+int mg_process_create(const char* proc, const mg_params_t* params, mg_process_t** out);
+int mg_process_destroy(mg_process_t* p);
+
+/* K1+K2: device Philox4x32-10 + RAMBO (PAPER.md:39 Fig. 1b, :47).  Writes nevt phase-space points for the
+ * process (beams along +-z with energy sqrt_s/2, final state flat in n-body phase space, massive tops put
+ * on shell by the RAMBO rescaling) into momenta_dev (layout above).  Random stream: Philox key = seed,
+ * counter = (global event index, final-particle index), so event i is the same for any batch split.
+ * Asynchronous on `stream`. */
+int mg_rambo(mg_process_t* p, uint64_t seed, double sqrt_s, int64_t nevt, void* momenta_dev, void* stream);
+/* Same, for events [first_event, first_event + nevt) of the stream, optionally with RAMBO weights
+ * (weights_dev may be NULL; double[nevt]; phase-space weight without the (2 pi)^(4-3n) factor). */
+int mg_rambo_ex(mg_process_t* p, uint64_t seed, double sqrt_s, int64_t first_event, int64_t nevt,
+                void* momenta_dev, double* weights_dev, void* stream);
+
+/* K1 alone (diagnostic / bit-exact test entry): the raw Philox4x32-10 words RAMBO consumes,
+ * out_dev[(ievt * nfinal + ifinal) * 4 + m], uint32, 16-byte aligned.  Asynchronous on `stream`. */
+int mg_philox_raw(mg_process_t* p, uint64_t seed, int64_t first_event, int64_t nevt, uint32_t* out_dev, void* stream);
+
+/* K3..K7: |M|^2 for nevt events.  momenta_dev: layout above; me_out_dev: nevt doubles (MG_FP64) or floats
+ * (MG_FP32).  Asynchronous on `stream`, except that in MG_HEL_FILTER mode the first call runs the
+ * helicity probe (K8) on the first min(nevt, 4096) events and synchronises the stream once. */
+int mg_sigma(mg_process_t* p, const void* momenta_dev, int64_t nevt, void* me_out_dev, void* stream);
+
+/* Same from HOST buffers (momenta_host: layout above, me_out_host: nevt elements): copies in, runs, copies
+ * out and synchronises.  This is the end-to-end entry point bench.py times as `e2e`. */
+int mg_sigma_host(mg_process_t* p, const void* momenta_host, int64_t nevt, void* me_out_host, void* stream);
+
+/* K8: explicit helicity probe on nprobe events; sets the good-helicity list (synchronises). */
+int mg_helicity_probe(mg_process_t* p, const void* momenta_dev, int64_t nprobe, void* stream);
+/* Per-helicity |M_h|^2 (already divided by the denominator), all 2^npar helicities:
+ * perhel_out_dev[h * nevt + ievt].  Diagnostic / test entry point. */
+int mg_sigma_per_helicity(mg_process_t* p, const void* momenta_dev, int64_t nevt, void* perhel_out_dev,
+                          void* stream);
+/* Copies the current good-helicity list (indices; bit (npar-1-i) set <=> particle i has lambda=+1). */
+int mg_good_helicities(const mg_process_t* p, int32_t* out, int32_t capacity, int32_t* ngood);
+
+int mg_process_info(const mg_process_t* p, mg_info_t* out);
+size_t mg_momenta_bytes(const mg_process_t* p, int64_t nevt);
+
+/* Measures the sustained FP64 (prec = MG_FP64) or FP32 FMA rate of the device with a dependent-chain-free
+ * FMA loop on every SM: the denominator of the "% of peak" figure.  Returns FLOP/s in
+ * *flops_per_s; synchronises. */
+int mg_fma_peak(int device, int prec, double* flops_per_s);
+
+const char* mg_status_string(int status);
+const char* mg_last_error(void); /* thread-local detail of the last MG_ERR_CUDA */
+
+#ifdef __cplusplus
+}
+#endif
+#endif

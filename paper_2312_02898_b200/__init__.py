@@ -1,0 +1,228 @@
+"""Thin Python binding of libmg5b200.so (include/mg5b200.h) — argument marshalling only.
+
+Every step of the path (Philox, RAMBO, wavefunctions, currents, amplitudes, colour sum, helicity sum) runs
+in the CUDA kernels behind the C ABI; PyTorch is used here only to own device buffers and streams.  There is
+no CPU fallback: importing works without a GPU (so the symbol table can be checked), but creating a process
+without a CUDA device raises.
+
+    proc = Process("g g > t t~ g g")
+    mom  = proc.rambo(seed=4, sqrt_s=1500.0, nevt=524288)      # torch.float64 CUDA tensor (AoSoA pages)
+    me   = proc.sigma(mom, nevt=524288)                         # torch tensor [nevt]
+"""
+import ctypes as C
+import os
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libmg5b200.so")
+NEPP = 32
+FP64, FP32 = 0, 1
+HEL_FILTER, HEL_ALL = 0, 1
+
+SYMBOLS = ["mg_params_default", "mg_process_create", "mg_process_destroy", "mg_rambo", "mg_rambo_ex", "mg_philox_raw", "mg_sigma",
+           "mg_sigma_host", "mg_helicity_probe", "mg_sigma_per_helicity", "mg_good_helicities", "mg_process_info",
+           "mg_momenta_bytes", "mg_fma_peak", "mg_status_string", "mg_last_error"]
+
+
+class MgParams(C.Structure):
+    _fields_ = [("struct_size", C.c_uint32), ("precision", C.c_int32), ("helicity_mode", C.c_int32),
+                ("device", C.c_int32), ("alpha_s", C.c_double), ("alpha_ew_inv", C.c_double), ("gf", C.c_double),
+                ("sw2", C.c_double), ("mz", C.c_double), ("gamma_z", C.c_double), ("mt", C.c_double),
+                ("gamma_t", C.c_double)]
+
+
+class MgInfo(C.Structure):
+    _fields_ = [("npar", C.c_int32), ("nfinal", C.c_int32), ("ndiagrams", C.c_int32), ("nhel", C.c_int32),
+                ("ngoodhel", C.c_int32), ("ncolor", C.c_int32), ("denominator", C.c_int32), ("nepp", C.c_int32),
+                ("flops_per_event_allhel", C.c_int64), ("flops_per_event_goodhel", C.c_int64),
+                ("masses", C.c_double * 8)]
+
+
+class MgError(RuntimeError):
+    def __init__(self, status, detail=""):
+        self.status = status
+        super().__init__("mg5b200 error %d (%s) %s" % (status, status_string(status), detail))
+
+
+_lib = None
+
+
+def lib():
+    """Loads the C-ABI library (fails loudly if it was not built: run `python -m paper_2312_02898_b200.build`)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError("libmg5b200.so not built; run `python -m paper_2312_02898_b200.build`")
+        L = C.CDLL(LIB_PATH)
+        vp, i64, u64 = C.c_void_p, C.c_int64, C.c_uint64
+        L.mg_params_default.argtypes = [C.POINTER(MgParams)]
+        L.mg_process_create.argtypes = [C.c_char_p, C.POINTER(MgParams), C.POINTER(vp)]
+        L.mg_process_destroy.argtypes = [vp]
+        L.mg_rambo.argtypes = [vp, u64, C.c_double, i64, vp, vp]
+        L.mg_rambo_ex.argtypes = [vp, u64, C.c_double, i64, i64, vp, vp, vp]
+        L.mg_philox_raw.argtypes = [vp, u64, i64, i64, vp, vp]
+        L.mg_sigma.argtypes = [vp, vp, i64, vp, vp]
+        L.mg_sigma_host.argtypes = [vp, vp, i64, vp, vp]
+        L.mg_helicity_probe.argtypes = [vp, vp, i64, vp]
+        L.mg_sigma_per_helicity.argtypes = [vp, vp, i64, vp, vp]
+        L.mg_good_helicities.argtypes = [vp, C.POINTER(C.c_int32), C.c_int32, C.POINTER(C.c_int32)]
+        L.mg_process_info.argtypes = [vp, C.POINTER(MgInfo)]
+        L.mg_momenta_bytes.argtypes = [vp, i64]
+        L.mg_momenta_bytes.restype = C.c_size_t
+        L.mg_fma_peak.argtypes = [C.c_int, C.c_int, C.POINTER(C.c_double)]
+        L.mg_status_string.argtypes = [C.c_int]
+        L.mg_status_string.restype = C.c_char_p
+        L.mg_last_error.restype = C.c_char_p
+        _lib = L
+    return _lib
+
+
+def status_string(status):
+    return lib().mg_status_string(status).decode()
+
+
+def _check(rc):
+    if rc != 0:
+        raise MgError(rc, lib().mg_last_error().decode() if rc == -7 else "")
+
+
+def default_params(precision=FP64, helicity_mode=HEL_FILTER, device=0, **kw):
+    p = MgParams()
+    _check(lib().mg_params_default(C.byref(p)))
+    p.precision, p.helicity_mode, p.device = precision, helicity_mode, device
+    for k, v in kw.items():
+        setattr(p, k, v)
+    return p
+
+
+def fma_peak(device=0, precision=FP64):
+    """Measured FMA rate (FLOP/s) of the device: the denominator of '% of FP64 peak'."""
+    out = C.c_double()
+    _check(lib().mg_fma_peak(device, precision, C.byref(out)))
+    return out.value
+
+
+def _stream_ptr(stream):
+    if stream is None:
+        import torch
+        stream = torch.cuda.current_stream()
+    return C.c_void_p(stream.cuda_stream)
+
+
+class Process:
+    """One process handle (mg_process_t)."""
+
+    def __init__(self, proc, precision=FP64, helicity_mode=HEL_FILTER, device=0, **params):
+        self._h = C.c_void_p()
+        self.params = default_params(precision, helicity_mode, device, **params)
+        self.proc = proc
+        _check(lib().mg_process_create(proc.encode(), C.byref(self.params), C.byref(self._h)))
+        self.precision = precision
+        self.device = device
+
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h.value:
+            lib().mg_process_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    @property
+    def info(self):
+        o = MgInfo()
+        _check(lib().mg_process_info(self._h, C.byref(o)))
+        return o
+
+    def momenta_bytes(self, nevt):
+        return int(lib().mg_momenta_bytes(self._h, nevt))
+
+    def alloc_momenta(self, nevt):
+        import torch
+        return torch.empty(self.momenta_bytes(nevt) // 8, dtype=torch.float64, device="cuda:%d" % self.device)
+
+    def rambo(self, seed, sqrt_s, nevt, first_event=0, out=None, weights=False, stream=None):
+        """mg_rambo / mg_rambo_ex -> AoSoA momenta tensor (and weights)."""
+        import torch
+        mom = out if out is not None else self.alloc_momenta(nevt)
+        w = torch.empty(nevt, dtype=torch.float64, device=mom.device) if weights else None
+        _check(lib().mg_rambo_ex(self._h, seed, float(sqrt_s), first_event, nevt, C.c_void_p(mom.data_ptr()),
+                                 C.c_void_p(w.data_ptr()) if weights else None, _stream_ptr(stream)))
+        return (mom, w) if weights else mom
+
+    def philox_raw(self, seed, nevt, first_event=0, stream=None):
+        """mg_philox_raw -> int32 tensor [nevt, nfinal, 4] holding the raw uint32 words."""
+        import torch
+        nf = self.info.nfinal
+        out = torch.empty((nevt, nf, 4), dtype=torch.int32, device="cuda:%d" % self.device)
+        _check(lib().mg_philox_raw(self._h, seed, first_event, nevt, C.c_void_p(out.data_ptr()), _stream_ptr(stream)))
+        return out
+
+    def _out_dtype(self):
+        import torch
+        return torch.float64 if self.precision == FP64 else torch.float32
+
+    def sigma(self, momenta, nevt, out=None, stream=None):
+        """mg_sigma: |M|^2 per event (device tensor in, device tensor out)."""
+        import torch
+        assert momenta.is_cuda and momenta.dtype == torch.float64 and momenta.numel() * 8 >= self.momenta_bytes(nevt)
+        me = out if out is not None else torch.empty(nevt, dtype=self._out_dtype(), device=momenta.device)
+        _check(lib().mg_sigma(self._h, C.c_void_p(momenta.data_ptr()), nevt, C.c_void_p(me.data_ptr()),
+                              _stream_ptr(stream)))
+        return me
+
+    def sigma_host(self, momenta_host, nevt, out_host=None, stream=None):
+        """mg_sigma_host: host (ideally pinned) tensors in and out; includes H2D/D2H copies."""
+        import torch
+        assert not momenta_host.is_cuda and momenta_host.dtype == torch.float64
+        me = out_host if out_host is not None else torch.empty(nevt, dtype=self._out_dtype()).pin_memory()
+        _check(lib().mg_sigma_host(self._h, C.c_void_p(momenta_host.data_ptr()), nevt, C.c_void_p(me.data_ptr()),
+                                   _stream_ptr(stream)))
+        return me
+
+    def sigma_per_helicity(self, momenta, nevt, stream=None):
+        import torch
+        nhel = self.info.nhel
+        out = torch.empty((nhel, nevt), dtype=self._out_dtype(), device=momenta.device)
+        _check(lib().mg_sigma_per_helicity(self._h, C.c_void_p(momenta.data_ptr()), nevt, C.c_void_p(out.data_ptr()),
+                                           _stream_ptr(stream)))
+        return out
+
+    def helicity_probe(self, momenta, nprobe, stream=None):
+        _check(lib().mg_helicity_probe(self._h, C.c_void_p(momenta.data_ptr()), nprobe, _stream_ptr(stream)))
+        return self.good_helicities()
+
+    def good_helicities(self):
+        n = C.c_int32()
+        buf = (C.c_int32 * 256)()
+        _check(lib().mg_good_helicities(self._h, buf, 256, C.byref(n)))
+        return [int(buf[i]) for i in range(n.value)]
+
+
+def pages_to_events(momenta, nevt, npar):
+    """AoSoA pages [page][ipar][32][4] -> plain [nevt][npar][4] (layout shuffle only; torch or numpy)."""
+    pages = (nevt + NEPP - 1) // NEPP
+    v = momenta[: pages * npar * NEPP * 4].reshape(pages, npar, NEPP, 4)
+    if hasattr(v, "permute"):
+        return v.permute(0, 2, 1, 3).reshape(pages * NEPP, npar, 4)[:nevt]
+    return v.transpose(0, 2, 1, 3).reshape(pages * NEPP, npar, 4)[:nevt]
+
+
+def events_to_pages(events):
+    """Plain [nevt][npar][4] (numpy or torch) -> AoSoA pages, zero-padded to whole pages."""
+    import numpy as np
+    is_torch = hasattr(events, "permute")
+    ev = events.cpu().numpy() if is_torch else np.asarray(events, dtype=np.float64)
+    nevt, npar, _ = ev.shape
+    pages = (nevt + NEPP - 1) // NEPP
+    buf = np.zeros((pages * NEPP, npar, 4))
+    buf[:nevt] = ev
+    if nevt < pages * NEPP:          # pad with copies of the last event so tail lanes stay finite
+        buf[nevt:] = ev[-1] if nevt else 0.0
+    out = np.ascontiguousarray(buf.reshape(pages, NEPP, npar, 4).transpose(0, 2, 1, 3)).reshape(-1)
+    if is_torch:
+        import torch
+        return torch.from_numpy(out)
+    return out

@@ -1,0 +1,88 @@
+"""Build step: run the process generator (K0) and compile libmg5b200.so for sm_100a, in-tree.
+
+    python -m paper_2312_02898_b200.build [--force]
+
+Generated sources go to csrc/generated/ (git-ignored: they are a pure function of gen/); objects to
+csrc/build/; the shared library next to this file.  nvcc cross-compiles without a GPU.
+"""
+import hashlib
+import os
+import subprocess
+import sys
+from concurrent.futures import ThreadPoolExecutor
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+CSRC = os.path.join(HERE, "csrc")
+GEN = os.path.join(CSRC, "generated")
+OBJ = os.path.join(CSRC, "build")
+LIB = os.path.join(HERE, "libmg5b200.so")
+NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
+FLAGS = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", "-I", CSRC]
+
+
+def generate():
+    from .gen.emit import emit_eemumu, emit_ggttng
+    os.makedirs(GEN, exist_ok=True)
+    infos, paths = [], []
+    jobs = [emit_eemumu()] + [emit_ggttng(n, fp32=(n < 5)) for n in (2, 3, 4, 5)]
+    for src, info in jobs:
+        path = os.path.join(GEN, info["ns"] + ".cu")
+        old = open(path).read() if os.path.exists(path) else None
+        if old != src:
+            with open(path, "w") as fh:
+                fh.write(src)
+        infos.append(info)
+        paths.append(path)
+    return paths, infos
+
+
+def _stamp(path):
+    h = hashlib.sha1()
+    for p in [path] + [os.path.join(CSRC, f) for f in sorted(os.listdir(CSRC)) if f.endswith((".cuh", ".h"))]:
+        with open(p, "rb") as fh:
+            h.update(fh.read())
+    with open(os.path.join(HERE, "..", "include", "mg5b200.h"), "rb") as fh:
+        h.update(fh.read())
+    h.update(" ".join(ARCH + FLAGS).encode())
+    return h.hexdigest()
+
+
+def _compile(path, force, log):
+    os.makedirs(OBJ, exist_ok=True)
+    base = os.path.splitext(os.path.basename(path))[0]
+    obj = os.path.join(OBJ, base + ".o")
+    stamp_file = obj + ".stamp"
+    stamp = _stamp(path)
+    if not force and os.path.exists(obj) and os.path.exists(stamp_file) and open(stamp_file).read() == stamp:
+        return obj
+    cmd = [NVCC] + ARCH + FLAGS + ["-Xptxas", "-v", "-c", path, "-o", obj]
+    r = subprocess.run(cmd, capture_output=True, text=True)
+    with open(os.path.join(OBJ, base + ".ptxas.log"), "w") as fh:
+        fh.write(" ".join(cmd) + "\n" + r.stdout + r.stderr)
+    if r.returncode != 0:
+        raise RuntimeError("nvcc failed for %s:\n%s" % (path, r.stderr[-4000:]))
+    with open(stamp_file, "w") as fh:
+        fh.write(stamp)
+    if log:
+        print("compiled", base, flush=True)
+    return obj
+
+
+def build(force=False, log=True):
+    gen_paths, infos = generate()
+    hand = [os.path.join(CSRC, f) for f in ("mg_api.cu", "mg_rambo.cu", "mg_peak.cu")]
+    srcs = gen_paths[::-1] + hand    # largest first
+    with ThreadPoolExecutor(max_workers=min(8, os.cpu_count() or 1)) as ex:
+        objs = list(ex.map(lambda p: _compile(p, force, log), srcs))
+    newest = max(os.path.getmtime(o) for o in objs)
+    if force or not os.path.exists(LIB) or os.path.getmtime(LIB) < newest:
+        cmd = [NVCC] + ARCH + ["-shared", "-o", LIB] + objs + ["-lcudart"]
+        subprocess.check_call(cmd)
+        if log:
+            print("linked", LIB, flush=True)
+    return LIB
+
+
+if __name__ == "__main__":
+    build(force="--force" in sys.argv)

@@ -1,0 +1,286 @@
+// mg_api.cu — the C ABI of include/mg5b200.h: argument checking, handle management, helicity filter (K8),
+// and dispatch to the generated per-process launchers.  No arithmetic of the method lives here.
+#include <math.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+#include <string>
+#include <vector>
+
+#include "../../include/mg5b200.h"
+#include "mg_internal.h"
+#include "mg_kernel.cuh"
+
+extern const mg_procdesc_t mg_desc_eemumu, mg_desc_ggtt, mg_desc_ggttg, mg_desc_ggttgg, mg_desc_ggttggg;
+static const mg_procdesc_t* const kProcs[] = {&mg_desc_eemumu, &mg_desc_ggtt, &mg_desc_ggttg, &mg_desc_ggttgg,
+                                              &mg_desc_ggttggg};
+
+static thread_local char g_err[512] = "";
+static int cuda_fail(cudaError_t e, const char* where) {
+  snprintf(g_err, sizeof g_err, "%s: %s", where, cudaGetErrorString(e));
+  return MG_ERR_CUDA;
+}
+#define MG_CUDA(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cuda_fail(e_, #call); } while (0)
+
+struct mg_process {
+  const mg_procdesc_t* desc;
+  mg_params_t par;
+  double pvec[MG_NPAR_VEC];
+  double masses[8];
+  int nfinal;
+  int* hel_dev;            // good-helicity list on the device (nhel ints)
+  int* hel_all_dev;        // 0..nhel-1
+  std::vector<int> good;
+  bool probed;
+};
+
+static std::string squeeze(const char* s) {
+  std::string o;
+  for (; *s; ++s) if (!isspace((unsigned char)*s)) o.push_back(*s);
+  return o;
+}
+
+extern "C" {
+
+int mg_params_default(mg_params_t* p) {
+  if (!p) return MG_ERR_NULL;
+  memset(p, 0, sizeof *p);
+  p->struct_size = sizeof(mg_params_t);
+  p->precision = MG_FP64; p->helicity_mode = MG_HEL_FILTER; p->device = 0;
+  p->alpha_s = 0.118; p->alpha_ew_inv = 132.507; p->gf = 1.16639e-5; p->sw2 = 0.0;
+  p->mz = 91.188; p->gamma_z = 2.4414; p->mt = 173.0; p->gamma_t = 0.0;
+  return MG_OK;
+}
+
+int mg_process_create(const char* proc, const mg_params_t* params, mg_process_t** out) {
+  if (!proc || !params || !out) return MG_ERR_NULL;
+  *out = nullptr;
+  if (params->struct_size != sizeof(mg_params_t)) return MG_ERR_BAD_PARAM;
+  if (params->precision != MG_FP64 && params->precision != MG_FP32) return MG_ERR_BAD_PARAM;
+  if (params->helicity_mode != MG_HEL_FILTER && params->helicity_mode != MG_HEL_ALL) return MG_ERR_BAD_PARAM;
+  if (!(params->alpha_s > 0) || !(params->alpha_ew_inv > 0) || !(params->mz > 0) || !(params->mt >= 0) ||
+      params->gamma_t != 0.0)
+    return MG_ERR_BAD_PARAM;
+  const std::string key = squeeze(proc);
+  const mg_procdesc_t* d = nullptr;
+  for (const mg_procdesc_t* c : kProcs) if (squeeze(c->proc) == key) d = c;
+  if (!d) return MG_ERR_BAD_PROC;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev <= 0 || params->device < 0 || params->device >= ndev) {
+    cudaGetLastError();
+    return MG_ERR_NO_DEVICE;
+  }
+  MG_CUDA(cudaSetDevice(params->device));
+  mg_process* p = new mg_process();
+  p->desc = d; p->par = *params; p->probed = false;
+  p->nfinal = d->npar - 2;
+  for (int i = 0; i < 8; ++i) p->masses[i] = (i < d->npar && d->massive[i]) ? params->mt : 0.0;
+  // derived couplings (DESIGN.md §3 C2, reading A1)
+  const double pi = 3.14159265358979323846;
+  const double aew = 1.0 / params->alpha_ew_inv;
+  double sw2 = params->sw2;
+  if (!(sw2 > 0)) {
+    const double mz2 = params->mz * params->mz;
+    const double mw2 = mz2 / 2 + sqrt(mz2 * mz2 / 4 - pi * aew * mz2 / (sqrt(2.0) * params->gf));
+    sw2 = 1.0 - mw2 / mz2;
+  }
+  const double e2 = 4 * pi * aew, e = sqrt(e2);
+  const double gz = e / (2 * sqrt(sw2 * (1 - sw2))), gv = -0.5 + 2 * sw2, ga = -0.5;
+  memset(p->pvec, 0, sizeof p->pvec);
+  p->pvec[MG_PAR_GS2] = 4 * pi * params->alpha_s;
+  p->pvec[MG_PAR_MT] = params->mt;
+  p->pvec[MG_PAR_E2] = e2;
+  p->pvec[MG_PAR_GL] = -gz * (gv + ga);
+  p->pvec[MG_PAR_GR] = -gz * (gv - ga);
+  p->pvec[MG_PAR_MZ2] = params->mz * params->mz;
+  p->pvec[MG_PAR_MZGZ] = params->mz * params->gamma_z;
+  std::vector<int> all(d->nhel);
+  for (int h = 0; h < d->nhel; ++h) all[h] = h;
+  p->good = all;
+  cudaError_t e1 = cudaMalloc(&p->hel_dev, sizeof(int) * d->nhel);
+  cudaError_t e2c = e1 == cudaSuccess ? cudaMalloc(&p->hel_all_dev, sizeof(int) * d->nhel) : e1;
+  if (e2c != cudaSuccess) { delete p; return cuda_fail(e2c, "cudaMalloc(helicity list)"); }
+  cudaMemcpy(p->hel_dev, all.data(), sizeof(int) * d->nhel, cudaMemcpyHostToDevice);
+  cudaMemcpy(p->hel_all_dev, all.data(), sizeof(int) * d->nhel, cudaMemcpyHostToDevice);
+  if (params->helicity_mode == MG_HEL_ALL) p->probed = true;
+  *out = p;
+  return MG_OK;
+}
+
+int mg_process_destroy(mg_process_t* p) {
+  if (!p) return MG_ERR_NULL;
+  cudaSetDevice(p->par.device);
+  cudaFree(p->hel_dev);
+  cudaFree(p->hel_all_dev);
+  delete p;
+  return MG_OK;
+}
+
+size_t mg_momenta_bytes(const mg_process_t* p, int64_t nevt) {
+  if (!p || nevt < 0) return 0;
+  const int64_t pages = (nevt + MG_NEPP - 1) / MG_NEPP;
+  return (size_t)pages * p->desc->npar * MG_NEPP * 4 * sizeof(double);
+}
+
+int mg_rambo_ex(mg_process_t* p, uint64_t seed, double sqrt_s, int64_t first_event, int64_t nevt,
+                void* momenta_dev, double* weights_dev, void* stream) {
+  if (!p || (!momenta_dev && nevt > 0)) return MG_ERR_NULL;
+  if (nevt < 0 || first_event < 0) return MG_ERR_BAD_NEVT;
+  if (((uintptr_t)momenta_dev & 15) || ((uintptr_t)weights_dev & 7)) return MG_ERR_ALIGN;
+  double sm = 0;
+  for (int f = 0; f < p->nfinal; ++f) sm += p->masses[2 + f];
+  if (!(sqrt_s > sm)) return MG_ERR_KINEMATICS;
+  MG_CUDA(cudaSetDevice(p->par.device));
+  MG_CUDA(mg_launch_rambo(p->nfinal, p->masses + 2, sqrt_s, seed, first_event, nevt, (double*)momenta_dev, weights_dev,
+                          (cudaStream_t)stream));
+  return MG_OK;
+}
+int mg_rambo(mg_process_t* p, uint64_t seed, double sqrt_s, int64_t nevt, void* momenta_dev, void* stream) {
+  return mg_rambo_ex(p, seed, sqrt_s, 0, nevt, momenta_dev, nullptr, stream);
+}
+
+int mg_philox_raw(mg_process_t* p, uint64_t seed, int64_t first_event, int64_t nevt, uint32_t* out_dev, void* stream) {
+  if (!p || (!out_dev && nevt > 0)) return MG_ERR_NULL;
+  if (nevt < 0 || first_event < 0) return MG_ERR_BAD_NEVT;
+  if ((uintptr_t)out_dev & 15) return MG_ERR_ALIGN;
+  MG_CUDA(cudaSetDevice(p->par.device));
+  MG_CUDA(mg_launch_philox_raw(seed, first_event, nevt, p->nfinal, out_dev, (cudaStream_t)stream));
+  return MG_OK;
+}
+
+static size_t esize(const mg_process_t* p) { return p->par.precision == MG_FP64 ? 8 : 4; }
+
+int mg_sigma_per_helicity(mg_process_t* p, const void* momenta_dev, int64_t nevt, void* perhel_out_dev, void* stream) {
+  if (!p || ((!momenta_dev || !perhel_out_dev) && nevt > 0)) return MG_ERR_NULL;
+  if (nevt < 0) return MG_ERR_BAD_NEVT;
+  if (((uintptr_t)momenta_dev & 15) || ((uintptr_t)perhel_out_dev & 7)) return MG_ERR_ALIGN;
+  if (nevt == 0) return MG_OK;
+  MG_CUDA(cudaSetDevice(p->par.device));
+  void* tmp = nullptr;
+  MG_CUDA(cudaMalloc(&tmp, esize(p) * (size_t)nevt));
+  p->desc->launch(p->par.precision, (const double*)momenta_dev, tmp, nevt, p->hel_all_dev, p->desc->nhel,
+                  perhel_out_dev, p->pvec, (cudaStream_t)stream);
+  cudaError_t e = cudaGetLastError();
+  if (e == cudaSuccess) e = cudaStreamSynchronize((cudaStream_t)stream);
+  cudaFree(tmp);
+  if (e != cudaSuccess) return cuda_fail(e, "sigma_per_helicity");
+  return MG_OK;
+}
+
+int mg_helicity_probe(mg_process_t* p, const void* momenta_dev, int64_t nprobe, void* stream) {
+  if (!p || !momenta_dev) return MG_ERR_NULL;
+  if (nprobe <= 0) return MG_ERR_BAD_NEVT;
+  const int nhel = p->desc->nhel;
+  void* ph = nullptr;
+  MG_CUDA(cudaSetDevice(p->par.device));
+  MG_CUDA(cudaMalloc(&ph, esize(p) * (size_t)nprobe * nhel));
+  int rc = mg_sigma_per_helicity(p, momenta_dev, nprobe, ph, stream);
+  if (rc != MG_OK) { cudaFree(ph); return rc; }
+  std::vector<double> sum(nhel, 0.0);
+  if (p->par.precision == MG_FP64) {
+    std::vector<double> h((size_t)nprobe * nhel);
+    cudaMemcpy(h.data(), ph, sizeof(double) * h.size(), cudaMemcpyDeviceToHost);
+    for (int ih = 0; ih < nhel; ++ih) for (int64_t i = 0; i < nprobe; ++i) sum[ih] += h[(size_t)ih * nprobe + i];
+  } else {
+    std::vector<float> h((size_t)nprobe * nhel);
+    cudaMemcpy(h.data(), ph, sizeof(float) * h.size(), cudaMemcpyDeviceToHost);
+    for (int ih = 0; ih < nhel; ++ih) for (int64_t i = 0; i < nprobe; ++i) sum[ih] += h[(size_t)ih * nprobe + i];
+  }
+  cudaFree(ph);
+  double tot = 0;
+  for (double s : sum) tot += s;
+  // reading A6: h is good iff sum_probe ME_h > eps * sum_probe sum_h ME_h
+  const double eps = p->par.precision == MG_FP64 ? 1e-14 : 1e-6;
+  p->good.clear();
+  for (int ih = 0; ih < nhel; ++ih) if (sum[ih] > eps * tot) p->good.push_back(ih);
+  if (p->good.empty()) for (int ih = 0; ih < nhel; ++ih) p->good.push_back(ih);
+  MG_CUDA(cudaMemcpy(p->hel_dev, p->good.data(), sizeof(int) * p->good.size(), cudaMemcpyHostToDevice));
+  p->probed = true;
+  return MG_OK;
+}
+
+int mg_sigma(mg_process_t* p, const void* momenta_dev, int64_t nevt, void* me_out_dev, void* stream) {
+  if (!p || ((!momenta_dev || !me_out_dev) && nevt > 0)) return MG_ERR_NULL;
+  if (nevt < 0) return MG_ERR_BAD_NEVT;
+  if (((uintptr_t)momenta_dev & 15) || ((uintptr_t)me_out_dev & (esize(p) - 1))) return MG_ERR_ALIGN;
+  if (nevt == 0) return MG_OK;
+  MG_CUDA(cudaSetDevice(p->par.device));
+  if (!p->probed) {
+    int rc = mg_helicity_probe(p, momenta_dev, nevt < 4096 ? nevt : 4096, stream);
+    if (rc != MG_OK) return rc;
+  }
+  p->desc->launch(p->par.precision, (const double*)momenta_dev, me_out_dev, nevt, p->hel_dev, (int)p->good.size(),
+                  nullptr, p->pvec, (cudaStream_t)stream);
+  MG_CUDA(cudaGetLastError());
+  return MG_OK;
+}
+
+int mg_sigma_host(mg_process_t* p, const void* momenta_host, int64_t nevt, void* me_out_host, void* stream) {
+  if (!p || ((!momenta_host || !me_out_host) && nevt > 0)) return MG_ERR_NULL;
+  if (nevt < 0) return MG_ERR_BAD_NEVT;
+  if (nevt == 0) return MG_OK;
+  MG_CUDA(cudaSetDevice(p->par.device));
+  cudaStream_t st = (cudaStream_t)stream;
+  void *dm = nullptr, *dout = nullptr;
+  const size_t mb = mg_momenta_bytes(p, nevt);
+  MG_CUDA(cudaMallocAsync(&dm, mb, st));
+  cudaError_t e = cudaMallocAsync(&dout, esize(p) * (size_t)nevt, st);
+  if (e != cudaSuccess) { cudaFreeAsync(dm, st); return cuda_fail(e, "cudaMallocAsync"); }
+  int rc = MG_OK;
+  e = cudaMemcpyAsync(dm, momenta_host, mb, cudaMemcpyHostToDevice, st);
+  if (e == cudaSuccess) rc = mg_sigma(p, dm, nevt, dout, stream);
+  if (e == cudaSuccess && rc == MG_OK) e = cudaMemcpyAsync(me_out_host, dout, esize(p) * (size_t)nevt, cudaMemcpyDeviceToHost, st);
+  cudaFreeAsync(dm, st);
+  cudaFreeAsync(dout, st);
+  cudaError_t es = cudaStreamSynchronize(st);
+  if (rc != MG_OK) return rc;
+  if (e != cudaSuccess) return cuda_fail(e, "mg_sigma_host copy");
+  if (es != cudaSuccess) return cuda_fail(es, "mg_sigma_host sync");
+  return MG_OK;
+}
+
+int mg_good_helicities(const mg_process_t* p, int32_t* out, int32_t capacity, int32_t* ngood) {
+  if (!p || !ngood) return MG_ERR_NULL;
+  *ngood = (int32_t)p->good.size();
+  if (out) for (int i = 0; i < capacity && i < (int)p->good.size(); ++i) out[i] = p->good[i];
+  return MG_OK;
+}
+
+int mg_process_info(const mg_process_t* p, mg_info_t* o) {
+  if (!p || !o) return MG_ERR_NULL;
+  const mg_procdesc_t* d = p->desc;
+  o->npar = d->npar; o->nfinal = d->npar - 2; o->ndiagrams = d->ndiagrams; o->nhel = d->nhel;
+  o->ngoodhel = (int)p->good.size(); o->ncolor = d->ncol; o->denominator = d->denominator; o->nepp = MG_NEPP;
+  o->flops_per_event_allhel = d->flops_per_helicity * d->nhel;
+  o->flops_per_event_goodhel = d->flops_per_helicity * (long long)p->good.size();
+  for (int i = 0; i < 8; ++i) o->masses[i] = p->masses[i];
+  return MG_OK;
+}
+
+int mg_fma_peak(int device, int prec, double* flops_per_s) {
+  if (!flops_per_s) return MG_ERR_NULL;
+  if (prec != MG_FP64 && prec != MG_FP32) return MG_ERR_BAD_PARAM;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) { cudaGetLastError(); return MG_ERR_NO_DEVICE; }
+  MG_CUDA(cudaSetDevice(device));
+  MG_CUDA(mg_run_fma_peak(prec, flops_per_s));
+  return MG_OK;
+}
+
+const char* mg_status_string(int s) {
+  switch (s) {
+    case MG_OK: return "ok";
+    case MG_ERR_NULL: return "null pointer argument";
+    case MG_ERR_BAD_PROC: return "unknown process string";
+    case MG_ERR_BAD_PARAM: return "bad parameter struct";
+    case MG_ERR_BAD_NEVT: return "bad event count";
+    case MG_ERR_ALIGN: return "misaligned device pointer";
+    case MG_ERR_KINEMATICS: return "sqrt_s not above the final-state mass threshold";
+    case MG_ERR_CUDA: return "CUDA error";
+    case MG_ERR_NO_DEVICE: return "no CUDA device";
+    default: return "unknown status";
+  }
+}
+const char* mg_last_error(void) { return g_err; }
+
+}  // extern "C"

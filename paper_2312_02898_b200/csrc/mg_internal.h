@@ -1,0 +1,16 @@
+// mg_internal.h — declarations shared by the hand-written translation units of libmg5b200.so.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+constexpr int MG_NEPP_I = 32;   // events per AoSoA page (== MG_NEPP of include/mg5b200.h)
+
+// parameter vector handed to every generated launch function
+enum { MG_PAR_GS2 = 0, MG_PAR_MT = 1, MG_PAR_E2 = 2, MG_PAR_GL = 3, MG_PAR_GR = 4, MG_PAR_MZ2 = 5, MG_PAR_MZGZ = 6,
+       MG_NPAR_VEC = 8 };
+
+cudaError_t mg_launch_rambo(int nfinal, const double* masses, double sqrt_s, uint64_t seed, long long first_event,
+                            long long nevt, double* mom, double* wgt, cudaStream_t st);
+cudaError_t mg_run_fma_peak(int prec, double* flops_per_s);
+cudaError_t mg_launch_philox_raw(uint64_t seed, long long first_event, long long nevt, int nfinal, uint32_t* out,
+                                 cudaStream_t st);

@@ -1,0 +1,58 @@
+// mg_peak.cu — FMA-rate micro-benchmark: the measured denominator of "% of FP64 (FP32) peak"
+// ("DFMA micro-benchmark peak measured on the same box in the same run").
+// 16 independent FMA chains per thread, 512 threads x 4 CTAs per SM, no memory traffic in the loop.
+#include "mg_internal.h"
+
+namespace {
+template <class T>
+__global__ void __launch_bounds__(512) fma_peak_kernel(T* out, int iters, T a, T b) {
+  T x[16];
+#pragma unroll
+  for (int k = 0; k < 16; ++k) x[k] = T(threadIdx.x + k) * T(1e-3);
+#pragma unroll 1
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int r = 0; r < 8; ++r) {
+#pragma unroll
+      for (int k = 0; k < 16; ++k) x[k] = x[k] * a + b;
+    }
+  }
+  T s = T(0);
+#pragma unroll
+  for (int k = 0; k < 16; ++k) s += x[k];
+  if (s == T(-1.2345)) out[blockIdx.x * blockDim.x + threadIdx.x] = s;   // never true; keeps the chain alive
+}
+
+template <class T> cudaError_t run(double* flops_per_s) {
+  int dev = 0, nsm = 0;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
+  const int block = 512, grid = nsm * 4 * 4;
+  const int iters = sizeof(T) == 8 ? 2000 : 8000;
+  T* out = nullptr;
+  cudaError_t e = cudaMalloc(&out, sizeof(T) * (size_t)block * grid);
+  if (e != cudaSuccess) return e;
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0); cudaEventCreate(&e1);
+  double best = 0;
+  for (int rep = 0; rep < 5; ++rep) {
+    cudaEventRecord(e0);
+    fma_peak_kernel<T><<<grid, block>>>(out, iters, T(0.999999), T(1e-7));
+    cudaEventRecord(e1);
+    e = cudaEventSynchronize(e1);
+    if (e != cudaSuccess) break;
+    float ms = 0;
+    cudaEventElapsedTime(&ms, e0, e1);
+    const double fl = 2.0 * 16 * 8 * (double)iters * block * (double)grid;
+    if (rep >= 1 && fl / (ms * 1e-3) > best) best = fl / (ms * 1e-3);
+  }
+  cudaEventDestroy(e0); cudaEventDestroy(e1);
+  cudaFree(out);
+  *flops_per_s = best;
+  return e != cudaSuccess ? e : cudaGetLastError();
+}
+}  // namespace
+
+cudaError_t mg_run_fma_peak(int prec, double* flops_per_s) {
+  return prec == 0 ? run<double>(flops_per_s) : run<float>(flops_per_s);
+}

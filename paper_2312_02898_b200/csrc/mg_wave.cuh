@@ -333,4 +333,25 @@ template <class T> MG_DEV C1<T> contract(const W4<T>& B, const W4<T>& j) {
   return d;
 }
 
+// Chiral halves of the bilinear (config 1, Z couplings):  BL_mu = L gamma_mu P_L R,  BR_mu = L gamma_mu P_R R
+// (P_L = upper two components in the Weyl basis); index lowered as in bilinear().
+template <class T> MG_DEV void bilinear_lr(const W4<T>& L, const W4<T>& R, W4<T>& BL, W4<T>& BR) {
+  C1<T> a0 = {L.r[0], L.i[0]}, a1 = {L.r[1], L.i[1]}, c0 = {L.r[2], L.i[2]}, c1 = {L.r[3], L.i[3]};
+  C1<T> d0 = {R.r[0], R.i[0]}, d1 = {R.r[1], R.i[1]}, b0 = {R.r[2], R.i[2]}, b1 = {R.r[3], R.i[3]};
+  T ab00r = MG_CMUL_R(a0, b0), ab00i = MG_CMUL_I(a0, b0), ab11r = MG_CMUL_R(a1, b1), ab11i = MG_CMUL_I(a1, b1);
+  T ab01r = MG_CMUL_R(a0, b1), ab01i = MG_CMUL_I(a0, b1), ab10r = MG_CMUL_R(a1, b0), ab10i = MG_CMUL_I(a1, b0);
+  T cd00r = MG_CMUL_R(c0, d0), cd00i = MG_CMUL_I(c0, d0), cd11r = MG_CMUL_R(c1, d1), cd11i = MG_CMUL_I(c1, d1);
+  T cd01r = MG_CMUL_R(c0, d1), cd01i = MG_CMUL_I(c0, d1), cd10r = MG_CMUL_R(c1, d0), cd10i = MG_CMUL_I(c1, d0);
+  BR.r[0] = ab00r + ab11r;      BR.i[0] = ab00i + ab11i;
+  BR.r[3] = -(ab00r - ab11r);   BR.i[3] = -(ab00i - ab11i);
+  BR.r[1] = -(ab01r + ab10r);   BR.i[1] = -(ab01i + ab10i);
+  BR.r[2] = -(ab01i - ab10i);   BR.i[2] = (ab01r - ab10r);
+  BL.r[0] = cd00r + cd11r;      BL.i[0] = cd00i + cd11i;
+  BL.r[3] = (cd00r - cd11r);    BL.i[3] = (cd00i - cd11i);
+  BL.r[1] = (cd01r + cd10r);    BL.i[1] = (cd01i + cd10i);
+  BL.r[2] = (cd01i - cd10i);    BL.i[2] = -(cd01r - cd10r);
+}
+// Minkowski product of two index-lowered complex vectors
+template <class T> MG_DEV C1<T> mink(const W4<T>& a, const W4<T>& b) { return wdot(a, b); }
+
 }  // namespace mgw
