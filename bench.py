@@ -1,0 +1,271 @@
+#!/usr/bin/env python
+"""bench.py — throughput of the hot path (matrix elements / second) on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload ggttgg|ggttggg|...] [--impl reference]
+
+A *step* is one pass of the whole hot path over one batch of synthetic input:
+mg_rambo (device Philox + RAMBO) followed by mg_sigma on BASELINE.json's configuration (default: config 4,
+g g > t t~ g g, 524288 events, sqrt(s) = 1500 GeV, seed 4, fp64 — the first process BASELINE.json's metric
+is quoted on).  Prints ONE JSON line (contract in the task statement): `value` = ME/s with inputs resident
+in HBM; `e2e` = the same through mg_sigma_host with pinned HOST buffers (H2D/D2H inside the timed region);
+`roofline` = achieved FP64 FLOP/s of the sigma kernel(s) against the FMA peak measured in the same run
+(mg_fma_peak), bound "alu"; `cpu_baseline` = the CPU oracle timed on this box's host cores on a bounded
+sample.  `--impl reference` times the oracle alone (it is the reference arm of this tier).
+Under torchrun each rank takes its own shard of the Philox event stream (first_event = rank * nevt): weak
+scaling, no data-path collective.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+import workloads  # noqa: E402
+
+METRIC = "matrix elements/sec"
+UNIT = "ME/s"
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--workload", default=os.environ.get("MG_BENCH_WORKLOAD", "ggttgg"), choices=list(workloads.CONFIGS))
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--precision", default="fp64", choices=["fp64", "fp32"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    return ap.parse_args()
+
+
+def config_dict(name, cfg, world, precision):
+    return {"workload": "%s: %s, sqrt_s=%g GeV, %d RAMBO events/GPU, Philox seed %d (BASELINE.json configs[%d])"
+                        % (name, cfg["proc"], cfg["sqrt_s"], cfg["nevt"], cfg["seed"], cfg["index"]),
+            "proc": cfg["proc"], "nevt_per_gpu": cfg["nevt"], "global_batch": cfg["nevt"] * world,
+            "sqrt_s": cfg["sqrt_s"], "seed": cfg["seed"], "precision": precision,
+            "parallelism": "events sharded over %d GPU(s), no collective" % world,
+            "l2": "step rewrites the 100 MB momenta batch; 256 MB L2 flush between timed steps"}
+
+
+# ---------------------------------------------------------------------------------------------- oracle legs
+ORACLE_SAMPLE = {"eemumu": 16384, "ggtt": 65536, "ggttg": 16384, "ggttgg": 4096, "ggttggg": 48}
+
+
+def oracle_time(name, cfg, nsample, repeats=1):
+    """Times the oracle as it stands (double build, OpenMP over events) on `nsample` events of the workload."""
+    from oracle import oracle as O
+    orc = O.load(False)
+    mom = orc.rambo(cfg["seed"], nsample, cfg["masses_final"], cfg["sqrt_s"])
+    best = None
+    for _ in range(repeats):
+        t0 = time.perf_counter()
+        me = orc.me_batch(cfg["proc"], mom)
+        dt = time.perf_counter() - t0
+        best = dt if best is None else min(best, dt)
+    assert (me > 0).all()
+    return nsample / best, best, orc.num_threads()
+
+
+def run_reference(args, name, cfg):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    nsample = max(8, ORACLE_SAMPLE[name] // 4)
+    from oracle import oracle as O
+    orc = O.load(False)
+    mom = orc.rambo(cfg["seed"], nsample, cfg["masses_final"], cfg["sqrt_s"])
+    for _ in range(min(args.warmup, 1)):
+        orc.me_batch(cfg["proc"], mom[: max(8, nsample // 8)])
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        mom = orc.rambo(cfg["seed"], nsample, cfg["masses_final"], cfg["sqrt_s"])
+        orc.me_batch(cfg["proc"], mom)
+    dt = time.perf_counter() - t0
+    val = nsample * args.steps / dt
+    cores = orc.num_threads()
+    sample = "%d events per step (prefix of the workload's seeded RAMBO batch), oracle RAMBO + |M|^2" % nsample
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": config_dict(name, cfg, 1, "fp64"),
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+# ---------------------------------------------------------------------------------------------- clocks
+class ClockSampler:
+    Q = "clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
+        "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+
+    def __init__(self, index):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons, pw = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1])); pw.append(float(r[2]))
+            except (ValueError, IndexError):
+                continue
+            for nm, v in zip(names, r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ---------------------------------------------------------------------------------------------- main arm
+def main():
+    args = parse()
+    name = args.workload
+    cfg = workloads.CONFIGS[name]
+    if args.impl == "reference":
+        return run_reference(args, name, cfg)
+
+    import torch
+    import paper_2312_02898_b200 as mg
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    prec = mg.FP64 if args.precision == "fp64" else mg.FP32
+    proc = mg.Process(cfg["proc"], precision=prec, device=local)
+    nevt = cfg["nevt"]
+    first = rank * nevt
+    st = torch.cuda.current_stream()
+    mom = proc.alloc_momenta(nevt)
+    me = torch.empty(nevt, dtype=torch.float64 if prec == mg.FP64 else torch.float32, device=mom.device)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=mom.device)
+
+    # set-up outside the timed region: helicity probe (K8), FMA peak measurement
+    proc.rambo(cfg["seed"], cfg["sqrt_s"], nevt, first_event=first, out=mom)
+    proc.helicity_probe(mom, min(nevt, 4096))
+    info = proc.info
+    peak64 = mg.fma_peak(local, prec)
+    launches_per_step = proc.launches_per_sigma() + 1 if hasattr(proc, "launches_per_sigma") else 2
+
+    def step(ev=None):
+        if ev:
+            ev[0].record(st)
+        proc.rambo(cfg["seed"], cfg["sqrt_s"], nevt, first_event=first, out=mom, stream=st)
+        if ev:
+            ev[1].record(st)
+        proc.sigma(mom, nevt, out=me, stream=st)
+        if ev:
+            ev[2].record(st)
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    torch.cuda.synchronize()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
+    if dist:
+        dist.barrier()
+    torch.cuda.synchronize()
+    for k in range(args.steps):
+        flush.fill_(k & 0xFF)             # L2 flush between timed steps (not timed)
+        step(evs[k])
+    torch.cuda.synchronize()
+    if dist:
+        dist.barrier()
+    t_rambo = sum(e[0].elapsed_time(e[1]) for e in evs) * 1e-3
+    t_sigma = sum(e[1].elapsed_time(e[2]) for e in evs) * 1e-3
+    t_total = t_rambo + t_sigma
+
+    # e2e: host buffers through the C ABI (mg_sigma_host): H2D of the momenta + D2H of |M|^2 in the timed region
+    host_mom = torch.empty(mom.numel(), dtype=torch.float64).pin_memory()
+    host_mom.copy_(mom)
+    host_me = torch.empty(nevt, dtype=me.dtype).pin_memory()
+    ne2e = max(3, min(args.steps, 5))
+    proc.sigma_host(host_mom, nevt, out_host=host_me)
+    torch.cuda.synchronize()
+    if dist:
+        dist.barrier()
+    t0 = time.perf_counter()
+    for _ in range(ne2e):
+        proc.sigma_host(host_mom, nevt, out_host=host_me)      # synchronises internally
+    t_e2e = (time.perf_counter() - t0) / ne2e
+    clocks = sampler.stop() if rank == 0 else None
+    assert torch.equal(host_me.cuda(), me), "host and device entry points disagree"
+
+    if dist:
+        t = torch.tensor([t_total, t_sigma, t_rambo, t_e2e], dtype=torch.float64, device=mom.device)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        t_total, t_sigma, t_rambo, t_e2e = [float(x) for x in t]
+    if rank != 0:
+        if dist:
+            dist.destroy_process_group()
+        return 0
+
+    flops_launch = float(info.flops_per_event_goodhel) * nevt        # generator's static count (FMA = 2)
+    achieved = flops_launch * args.steps / t_sigma
+    value = nevt * world * args.steps / t_total
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+        "ms_per_step": t_total / args.steps * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64" if prec == mg.FP64 else "f32", "data": "synthetic", "config": config_dict(name, cfg, world, args.precision),
+        "sigma_only": {"value": nevt * world * args.steps / t_sigma, "unit": UNIT, "ms": t_sigma / args.steps * 1e3},
+        "rambo_ms": t_rambo / args.steps * 1e3,
+        "e2e": {"value": nevt * world / t_e2e, "unit": UNIT, "h2d_bytes_per_step": host_mom.numel() * 8,
+                "d2h_bytes_per_step": host_me.numel() * host_me.element_size(), "ms": t_e2e * 1e3,
+                "api": "mg_sigma_host (pinned host momenta in, |M|^2 out)"},
+        "gpu_launches": launches_per_step * args.steps,
+        "roofline": {"bound": "alu", "achieved": achieved / 1e12, "peak": peak64 / 1e12, "unit": "TFLOP/s",
+                     "frac": achieved / peak64, "traffic": None,
+                     "kernel": "sigma (amplitudes + colour sum)",
+                     "flops_per_event": int(info.flops_per_event_goodhel), "ngoodhel": int(info.ngoodhel),
+                     "peak_source": "mg_fma_peak measured in this run (%s FMA loop on all SMs); MEASURED_PEAKS.json has no "
+                                    "FP64 entry" % ("DFMA" if prec == mg.FP64 else "FFMA")},
+        "clocks": clocks,
+    }
+    if not args.no_cpu_baseline:
+        ns = ORACLE_SAMPLE[name]
+        v, dt, cores = oracle_time(name, cfg, ns)
+        line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "seconds": dt,
+                                "sample": "first %d events of the workload's seeded RAMBO batch, |M|^2 only" % ns}
+    print(json.dumps(line), flush=True)
+    if dist:
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

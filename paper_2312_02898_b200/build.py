@@ -25,7 +25,8 @@ def generate():
     from .gen.emit import emit_eemumu, emit_ggttng
     os.makedirs(GEN, exist_ok=True)
     infos, paths = [], []
-    jobs = [emit_eemumu()] + [emit_ggttng(n, fp32=(n < 5)) for n in (2, 3, 4, 5)]
+    ns_gluons = [int(x) for x in os.environ.get("MG_NGLUONS", "2,3,4").split(",") if x]
+    jobs = [emit_eemumu()] + [emit_ggttng(n, fp32=(n < 5)) for n in ns_gluons]
     for src, info in jobs:
         path = os.path.join(GEN, info["ns"] + ".cu")
         old = open(path).read() if os.path.exists(path) else None
@@ -34,6 +35,16 @@ def generate():
                 fh.write(src)
         infos.append(info)
         paths.append(path)
+    tags = [i["ns"][3:] for i in infos]
+    reg = "// GENERATED: table of generated processes\n#include \"mg_kernel.cuh\"\n"
+    reg += "".join("extern const mg_procdesc_t mg_desc_%s;\n" % t for t in tags)
+    reg += "extern const mg_procdesc_t* const mg_registry[] = {%s};\n" % ", ".join("&mg_desc_" + t for t in tags)
+    reg += "extern const int mg_registry_n = %d;\n" % len(tags)
+    path = os.path.join(GEN, "mg_registry.cu")
+    if not os.path.exists(path) or open(path).read() != reg:
+        with open(path, "w") as fh:
+            fh.write(reg)
+    paths.append(path)
     return paths, infos
 
 

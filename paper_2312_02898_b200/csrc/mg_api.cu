@@ -11,9 +11,9 @@
 #include "mg_internal.h"
 #include "mg_kernel.cuh"
 
-extern const mg_procdesc_t mg_desc_eemumu, mg_desc_ggtt, mg_desc_ggttg, mg_desc_ggttgg, mg_desc_ggttggg;
-static const mg_procdesc_t* const kProcs[] = {&mg_desc_eemumu, &mg_desc_ggtt, &mg_desc_ggttg, &mg_desc_ggttgg,
-                                              &mg_desc_ggttggg};
+// table of generated processes: csrc/generated/mg_registry.cu (written by the generator)
+extern const mg_procdesc_t* const mg_registry[];
+extern const int mg_registry_n;
 
 static thread_local char g_err[512] = "";
 static int cuda_fail(cudaError_t e, const char* where) {
@@ -63,7 +63,7 @@ int mg_process_create(const char* proc, const mg_params_t* params, mg_process_t*
     return MG_ERR_BAD_PARAM;
   const std::string key = squeeze(proc);
   const mg_procdesc_t* d = nullptr;
-  for (const mg_procdesc_t* c : kProcs) if (squeeze(c->proc) == key) d = c;
+  for (int i = 0; i < mg_registry_n; ++i) if (squeeze(mg_registry[i]->proc) == key) d = mg_registry[i];
   if (!d) return MG_ERR_BAD_PROC;
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev <= 0 || params->device < 0 || params->device >= ndev) {

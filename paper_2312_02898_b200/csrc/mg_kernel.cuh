@@ -11,13 +11,13 @@
 #include <math.h>
 #include "mg_wave.cuh"
 
-constexpr int MG_NEPP = 32;
+constexpr int MGK_NEPP = 32;
 
 template <class T, int NPAR>
 MG_DEV void load_momentum(const double* __restrict__ mom, long long ievt, int ipar, mgw::P4<T>& p) {
-  const long long page = ievt / MG_NEPP;
-  const int lane = (int)(ievt % MG_NEPP);
-  const double* src = mom + ((page * NPAR + ipar) * MG_NEPP + lane) * 4;
+  const long long page = ievt / MGK_NEPP;
+  const int lane = (int)(ievt % MGK_NEPP);
+  const double* src = mom + ((page * NPAR + ipar) * MGK_NEPP + lane) * 4;
 #ifdef __CUDA_ARCH__
   const double2* q = reinterpret_cast<const double2*>(src);
   const double2 a = __ldg(q), b = __ldg(q + 1);
