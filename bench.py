@@ -52,7 +52,7 @@ def config_dict(name, cfg, world, precision):
 
 
 # ---------------------------------------------------------------------------------------------- oracle legs
-ORACLE_SAMPLE = {"eemumu": 16384, "ggtt": 65536, "ggttg": 16384, "ggttgg": 4096, "ggttggg": 48}
+ORACLE_SAMPLE = {"eemumu": 524288, "ggtt": 262144, "ggttg": 131072, "ggttgg": 49152, "ggttggg": 512}
 
 
 def oracle_time(name, cfg, nsample, repeats=1):
