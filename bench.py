@@ -39,6 +39,7 @@ def parse():
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--precision", default="fp64", choices=["fp64", "fp32"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--nevt", type=int, default=0, help="override the batch size (profiling runs only; not a bench value)")
     return ap.parse_args()
 
 
@@ -147,7 +148,9 @@ class ClockSampler:
 def main():
     args = parse()
     name = args.workload
-    cfg = workloads.CONFIGS[name]
+    cfg = dict(workloads.CONFIGS[name])
+    if args.nevt:
+        cfg["nevt"] = args.nevt
     if args.impl == "reference":
         return run_reference(args, name, cfg)
 

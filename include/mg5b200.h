@@ -69,6 +69,9 @@ typedef struct {
   int64_t flops_per_event_allhel;  /* generator's static FLOP count (FMA = 2), all helicities       */
   int64_t flops_per_event_goodhel; /* same for the current good-helicity list                       */
   double masses[8];                /* per particle, process order                                   */
+  int32_t nkernels_per_tile;       /* kernel launches mg_sigma makes per event tile (1 = fused kernel)      */
+  int32_t reserved;
+  int64_t workspace_bytes;         /* library-owned JAMP workspace currently allocated (split kernels only) */
 } mg_info_t;
 
 /* Fills *params with the defaults of BASELINE.json's configs (fp64, helicity filter, device 0). */
@@ -96,7 +99,10 @@ int mg_philox_raw(mg_process_t* p, uint64_t seed, int64_t first_event, int64_t n
 
 /* K3..K7: |M|^2 for nevt events.  momenta_dev: layout above; me_out_dev: nevt doubles (MG_FP64) or floats
  * (MG_FP32).  Asynchronous on `stream`, except that in MG_HEL_FILTER mode the first call runs the
- * helicity probe (K8) on the first min(nevt, 4096) events and synchronises the stream once. */
+ * helicity probe (K8) on the first min(nevt, 4096) events and synchronises the stream once, and that the
+ * processes with >= 24 colour flows keep partial JAMPs in a library-owned workspace (at most MG5B200_WS_GB
+ * GiB, default 8; larger batches are processed in event tiles) which is (re)allocated, synchronously, by
+ * the first call that needs a bigger one. */
 int mg_sigma(mg_process_t* p, const void* momenta_dev, int64_t nevt, void* me_out_dev, void* stream);
 
 /* Same from HOST buffers (momenta_host: layout above, me_out_host: nevt elements): copies in, runs, copies

@@ -22,19 +22,34 @@ FLAGS = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", "-I", CSRC]
 
 
 def generate():
+    """Runs the process generator; returns (list of generated .cu paths, list of info dicts)."""
+    import json
     from .gen.emit import emit_eemumu, emit_ggttng
     os.makedirs(GEN, exist_ok=True)
     infos, paths = [], []
-    ns_gluons = [int(x) for x in os.environ.get("MG_NGLUONS", "2,3,4").split(",") if x]
-    jobs = [emit_eemumu()] + [emit_ggttng(n, fp32=(n < 5)) for n in ns_gluons]
-    for src, info in jobs:
-        path = os.path.join(GEN, info["ns"] + ".cu")
-        old = open(path).read() if os.path.exists(path) else None
-        if old != src:
-            with open(path, "w") as fh:
-                fh.write(src)
+    ns_gluons = [int(x) for x in os.environ.get("MG_NGLUONS", "2,3,4,5").split(",") if x]
+    shapes = dict(kv.split("=") for kv in os.environ.get("MG_SHAPES", "").split(",") if kv)   # e.g. "4=fused"
+    maxterms = dict(kv.split("=") for kv in os.environ.get("MG_MAXTERMS", "").split(",") if kv)   # e.g. "4=40"
+    block = dict(kv.split("=") for kv in os.environ.get("MG_BLOCK", "").split(",") if kv)
+    jobs = [emit_eemumu()]
+    for n in ns_gluons:
+        kw = dict(fp32=(n < 5), acc_max=int(os.environ.get("MG_ACCMAX", "6")))
+        if str(n) in block:
+            kw["block"] = int(block[str(n)])
+        if str(n) in maxterms:
+            kw["max_terms"] = int(maxterms[str(n)])
+        jobs.append(emit_ggttng(n, shape=shapes.get(str(n)), **kw))
+    keep = set()
+    for files, info in jobs:
+        for fname, src in files:
+            path = os.path.join(GEN, fname)
+            old = open(path).read() if os.path.exists(path) else None
+            if old != src:
+                with open(path, "w") as fh:
+                    fh.write(src)
+            paths.append(path)
+            keep.add(fname)
         infos.append(info)
-        paths.append(path)
     tags = [i["ns"][3:] for i in infos]
     reg = "// GENERATED: table of generated processes\n#include \"mg_kernel.cuh\"\n"
     reg += "".join("extern const mg_procdesc_t mg_desc_%s;\n" % t for t in tags)
@@ -45,6 +60,12 @@ def generate():
         with open(path, "w") as fh:
             fh.write(reg)
     paths.append(path)
+    keep.add("mg_registry.cu")
+    for f in os.listdir(GEN):            # stale units of an earlier partition
+        if f.endswith(".cu") and f not in keep:
+            os.remove(os.path.join(GEN, f))
+    with open(os.path.join(GEN, "generator_info.json"), "w") as fh:
+        json.dump(infos, fh, indent=1, default=str)
     return paths, infos
 
 
@@ -83,7 +104,7 @@ def _compile(path, force, log):
 def build(force=False, log=True):
     gen_paths, infos = generate()
     hand = [os.path.join(CSRC, f) for f in ("mg_api.cu", "mg_rambo.cu", "mg_peak.cu")]
-    srcs = gen_paths[::-1] + hand    # largest first
+    srcs = sorted(gen_paths, key=lambda p: -os.path.getsize(p)) + hand    # largest first
     with ThreadPoolExecutor(max_workers=min(8, os.cpu_count() or 1)) as ex:
         objs = list(ex.map(lambda p: _compile(p, force, log), srcs))
     newest = max(os.path.getmtime(o) for o in objs)

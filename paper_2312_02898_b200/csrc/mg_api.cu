@@ -32,7 +32,30 @@ struct mg_process {
   int* hel_all_dev;        // 0..nhel-1
   std::vector<int> good;
   bool probed;
+  void* ws;                // workspace of the split kernel shape (JAMPs + per-helicity values), library-owned
+  size_t ws_bytes;
 };
+
+// Workspace for the split kernel shape: jamp[nhel_run][ncol][2][tile] + meh[nhel_run][tile]; the generated launcher
+// tiles the batch so that it fits.  Capped at MG5B200_WS_GB GiB (default 8).  Grows on demand (synchronous
+// cudaFree/cudaMalloc on the first call that needs more), never shrinks.
+static int ensure_ws(mg_process* p, int64_t nevt, int nhel_run) {
+  const int ip = p->par.precision == MG_FP64 ? 0 : 1;
+  const size_t bpe = (size_t)p->desc->ws_bytes_per_event_hel[ip] * (size_t)nhel_run + (size_t)p->desc->ws_bytes_per_event[ip];
+  if (bpe == 0) return MG_OK;
+  double cap_gb = 8.0;
+  if (const char* e = getenv("MG5B200_WS_GB")) { const double v = atof(e); if (v > 0) cap_gb = v; }
+  size_t cap = (size_t)(cap_gb * 1073741824.0);
+  if (cap < bpe * 1024) cap = bpe * 1024;
+  const size_t padded = (size_t)((nevt + 31) / 32 * 32);
+  size_t need = padded * bpe;
+  if (need > cap) need = cap / (bpe * 1024) * (bpe * 1024);
+  if (p->ws_bytes >= need) return MG_OK;
+  if (p->ws) { cudaDeviceSynchronize(); cudaFree(p->ws); p->ws = nullptr; p->ws_bytes = 0; }
+  MG_CUDA(cudaMalloc(&p->ws, need));
+  p->ws_bytes = need;
+  return MG_OK;
+}
 
 static std::string squeeze(const char* s) {
   std::string o;
@@ -56,7 +79,6 @@ int mg_process_create(const char* proc, const mg_params_t* params, mg_process_t*
   if (!proc || !params || !out) return MG_ERR_NULL;
   *out = nullptr;
   if (params->struct_size != sizeof(mg_params_t)) return MG_ERR_BAD_PARAM;
-  if (params->precision != MG_FP64 && params->precision != MG_FP32) return MG_ERR_BAD_PARAM;
   if (params->helicity_mode != MG_HEL_FILTER && params->helicity_mode != MG_HEL_ALL) return MG_ERR_BAD_PARAM;
   if (!(params->alpha_s > 0) || !(params->alpha_ew_inv > 0) || !(params->mz > 0) || !(params->mt >= 0) ||
       params->gamma_t != 0.0)
@@ -65,6 +87,7 @@ int mg_process_create(const char* proc, const mg_params_t* params, mg_process_t*
   const mg_procdesc_t* d = nullptr;
   for (int i = 0; i < mg_registry_n; ++i) if (squeeze(mg_registry[i]->proc) == key) d = mg_registry[i];
   if (!d) return MG_ERR_BAD_PROC;
+  if (params->precision != MG_FP64 && !(params->precision == MG_FP32 && d->has_fp32)) return MG_ERR_BAD_PARAM;
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev <= 0 || params->device < 0 || params->device >= ndev) {
     cudaGetLastError();
@@ -72,7 +95,7 @@ int mg_process_create(const char* proc, const mg_params_t* params, mg_process_t*
   }
   MG_CUDA(cudaSetDevice(params->device));
   mg_process* p = new mg_process();
-  p->desc = d; p->par = *params; p->probed = false;
+  p->desc = d; p->par = *params; p->probed = false; p->ws = nullptr; p->ws_bytes = 0;
   p->nfinal = d->npar - 2;
   for (int i = 0; i < 8; ++i) p->masses[i] = (i < d->npar && d->massive[i]) ? params->mt : 0.0;
   // derived couplings (DESIGN.md §3 C2, reading A1)
@@ -112,6 +135,7 @@ int mg_process_destroy(mg_process_t* p) {
   cudaSetDevice(p->par.device);
   cudaFree(p->hel_dev);
   cudaFree(p->hel_all_dev);
+  if (p->ws) cudaFree(p->ws);
   delete p;
   return MG_OK;
 }
@@ -157,9 +181,10 @@ int mg_sigma_per_helicity(mg_process_t* p, const void* momenta_dev, int64_t nevt
   if (nevt == 0) return MG_OK;
   MG_CUDA(cudaSetDevice(p->par.device));
   void* tmp = nullptr;
+  { const int rc = ensure_ws(p, nevt, p->desc->nhel); if (rc != MG_OK) return rc; }
   MG_CUDA(cudaMalloc(&tmp, esize(p) * (size_t)nevt));
   p->desc->launch(p->par.precision, (const double*)momenta_dev, tmp, nevt, p->hel_all_dev, p->desc->nhel,
-                  perhel_out_dev, p->pvec, (cudaStream_t)stream);
+                  perhel_out_dev, p->pvec, p->ws, p->ws_bytes, (cudaStream_t)stream);
   cudaError_t e = cudaGetLastError();
   if (e == cudaSuccess) e = cudaStreamSynchronize((cudaStream_t)stream);
   cudaFree(tmp);
@@ -209,8 +234,9 @@ int mg_sigma(mg_process_t* p, const void* momenta_dev, int64_t nevt, void* me_ou
     int rc = mg_helicity_probe(p, momenta_dev, nevt < 4096 ? nevt : 4096, stream);
     if (rc != MG_OK) return rc;
   }
+  { const int rc = ensure_ws(p, nevt, (int)p->good.size()); if (rc != MG_OK) return rc; }
   p->desc->launch(p->par.precision, (const double*)momenta_dev, me_out_dev, nevt, p->hel_dev, (int)p->good.size(),
-                  nullptr, p->pvec, (cudaStream_t)stream);
+                  nullptr, p->pvec, p->ws, p->ws_bytes, (cudaStream_t)stream);
   MG_CUDA(cudaGetLastError());
   return MG_OK;
 }
@@ -254,6 +280,9 @@ int mg_process_info(const mg_process_t* p, mg_info_t* o) {
   o->flops_per_event_allhel = d->flops_per_helicity * d->nhel;
   o->flops_per_event_goodhel = d->flops_per_helicity * (long long)p->good.size();
   for (int i = 0; i < 8; ++i) o->masses[i] = p->masses[i];
+  o->nkernels_per_tile = d->nkernels;
+  o->reserved = 0;
+  o->workspace_bytes = (int64_t)p->ws_bytes;
   return MG_OK;
 }
 

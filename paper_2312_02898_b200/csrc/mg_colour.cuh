@@ -1,0 +1,78 @@
+// mg_colour.cuh — K6 (colour sum) and K7 (helicity sum + averaging) for the split kernel shape
+// (north_star (4)).  Input: the JAMP workspace written by the diagram-group kernels,
+//     jamp[ih][flow][re/im][stride]   (element type T, event index fastest => coalesced),
+// output: me_out[evt] = norm * sum_ih  J^dagger CF J,  and optionally the per-helicity values.
+//
+// Register-blocked symmetric quadratic form: thread = one (event, helicity); for each block of 8 rows i the
+// thread keeps 8 complex partial sums z_i = CF_ii J_i + 2 sum_{j>i} CF_ij J_j in registers while J_j streams
+// in from L1/L2 (each J_j is re-read once per row block: ncol/16 times on average), then adds
+// Re(J_i^* z_i).  The coefficients come from a blocked upper-triangular table
+//     cf_table[block b][j >= 8b][8 rows]   (integers; the common denominator is folded into `norm`),
+// read with warp-uniform loads.  Half the FLOPs of the full matrix-vector product.
+#pragma once
+#include <cuda_runtime.h>
+
+namespace mgc {
+
+template <class T, int NCOL>
+__global__ void __launch_bounds__(128) colour_kernel(const double* __restrict__ cft, const T* __restrict__ jamp,
+                                                     T* __restrict__ meh, long long stride, long long nevt, int nhel_run) {
+  const long long ievt = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const int ih = blockIdx.y;
+  if (ievt >= nevt) return;
+  const T* __restrict__ jb = jamp + (long long)ih * (2 * NCOL) * stride + ievt;
+  T me = T(0);
+  const double* __restrict__ tab = cft;
+#pragma unroll 1
+  for (int i0 = 0; i0 < NCOL; i0 += 8) {
+    T zr[8], zi[8];
+#pragma unroll
+    for (int r = 0; r < 8; ++r) { zr[r] = T(0); zi[r] = T(0); }
+#pragma unroll 2
+    for (int j = i0; j < NCOL; ++j) {
+      const T jr = jb[(2 * j) * stride], ji = jb[(2 * j + 1) * stride];
+      const double2* c2 = reinterpret_cast<const double2*>(tab);
+#pragma unroll
+      for (int r = 0; r < 4; ++r) {
+        const double2 c = __ldg(c2 + r);
+        zr[2 * r] += T(c.x) * jr; zi[2 * r] += T(c.x) * ji;
+        zr[2 * r + 1] += T(c.y) * jr; zi[2 * r + 1] += T(c.y) * ji;
+      }
+      tab += 8;
+    }
+#pragma unroll
+    for (int r = 0; r < 8; ++r) {
+      if (i0 + r < NCOL) {
+        const T jr = jb[(2 * (i0 + r)) * stride], ji = jb[(2 * (i0 + r) + 1) * stride];
+        me += jr * zr[r] + ji * zi[r];
+      }
+    }
+  }
+  meh[(long long)ih * stride + ievt] = me;
+}
+
+// fixed-order helicity sum (deterministic), normalisation, optional per-helicity output
+template <class T>
+__global__ void helsum_kernel(const T* __restrict__ meh, long long stride, long long nevt, int nhel_run, T norm,
+                              T* __restrict__ me_out, T* __restrict__ perhel_out, long long perhel_stride) {
+  const long long ievt = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (ievt >= nevt) return;
+  T s = T(0);
+  for (int ih = 0; ih < nhel_run; ++ih) {
+    const T v = meh[(long long)ih * stride + ievt];
+    if (perhel_out) perhel_out[(long long)ih * perhel_stride + ievt] = v * norm;
+    s += v;
+  }
+  me_out[ievt] = s * norm;
+}
+
+template <class T, int NCOL>
+void colour_and_sum(const double* cft, const T* jamp, T* meh, long long stride, long long nevt, int nhel_run, double norm,
+                    T* me_out, T* perhel_out, long long perhel_stride, cudaStream_t st) {
+  const dim3 grid((unsigned)((nevt + 127) / 128), (unsigned)nhel_run);
+  colour_kernel<T, NCOL><<<grid, 128, 0, st>>>(cft, jamp, meh, stride, nevt, nhel_run);
+  helsum_kernel<T><<<(unsigned)((nevt + 255) / 256), 256, 0, st>>>(meh, stride, nevt, nhel_run, T(norm), me_out, perhel_out,
+                                                                   perhel_stride);
+}
+
+}  // namespace mgc

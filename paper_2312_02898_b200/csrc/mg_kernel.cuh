@@ -27,18 +27,43 @@ MG_DEV void load_momentum(const double* __restrict__ mom, long long ievt, int ip
 #endif
 }
 
+// Ordered loads/stores of the per-event invariants buffer inv[item][event] (split kernel shape).  asm volatile:
+// the compiler neither hoists these out of the helicity loop nor merges repeated loads, so helicity-independent
+// operands are fetched (L1/L2) where they are used instead of living in registers or spill slots.
+#ifdef __CUDA_ARCH__
+MG_DEV double ldv(const double* p) { double v; asm volatile("ld.global.ca.f64 %0, [%1];" : "=d"(v) : "l"(p)); return v; }
+MG_DEV float ldv(const float* p) { float v; asm volatile("ld.global.ca.f32 %0, [%1];" : "=f"(v) : "l"(p)); return v; }
+#else
+template <class T> MG_DEV T ldv(const T* p) { return *p; }
+#endif
+template <class T> MG_DEV mgw::P4<T> ldp(const T* p, long long stride) {
+  mgw::P4<T> o;
+#pragma unroll
+  for (int m = 0; m < 4; ++m) o.c[m] = ldv(p + m * stride);
+  return o;
+}
+template <class T> MG_DEV void stp(T* p, long long stride, const mgw::P4<T>& v) {
+#pragma unroll
+  for (int m = 0; m < 4; ++m) p[m * stride] = v.c[m];
+}
+
 template <int NPAR> MG_DEV int hel_of(int h, int ipar) {
   return ((h >> (NPAR - 1 - ipar)) & 1) ? 1 : -1;
 }
 
 #ifdef __CUDACC__
 typedef void (*mg_launch_fn)(int prec, const double* mom, void* me_out, long long nevt, const int* hel_list,
-                             int nhel_run, void* perhel_out, const double* par, cudaStream_t st);
+                             int nhel_run, void* perhel_out, const double* par, void* ws, size_t ws_bytes,
+                             cudaStream_t st);
 struct mg_procdesc_t {
   const char* proc;          // canonical process string
   int npar, ngluons, ndiagrams, nhel, ncol, denominator;
   long long flops_per_helicity;   // generator's static count (DFMA = 2)
   int massive[8];            // 1 where the particle has mass mt
   mg_launch_fn launch;
+  int ws_bytes_per_event_hel[2];  // workspace bytes per (event, helicity) for fp64 / fp32 (0: fused kernel)
+  int nkernels;              // kernel launches per event tile (diagram groups + colour + helicity sum)
+  int has_fp32;              // fp32 kernels were generated
+  int ws_bytes_per_event[2]; // workspace bytes per event (helicity-independent invariants) for fp64 / fp32
 };
 #endif  // __CUDACC__

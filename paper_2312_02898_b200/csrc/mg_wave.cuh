@@ -46,6 +46,12 @@ template <class T> MG_DEV P4<T> psub(const P4<T>& a, const P4<T>& b) {
   for (int m = 0; m < 4; ++m) o.c[m] = a.c[m] - b.c[m];
   return o;
 }
+template <class T, class S> MG_DEV P4<T> pcast(const P4<S>& a) {
+  P4<T> o;
+#pragma unroll
+  for (int m = 0; m < 4; ++m) o.c[m] = T(a.c[m]);
+  return o;
+}
 template <class T> MG_DEV T pdot(const P4<T>& a, const P4<T>& b) {
   return a.c[0] * b.c[0] - a.c[1] * b.c[1] - a.c[2] * b.c[2] - a.c[3] * b.c[3];
 }

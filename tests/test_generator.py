@@ -78,6 +78,34 @@ def test_plan_counts_and_recycling():
     for op in p4.ops:
         for nm in _inputs(op):
             assert nm in defined
-        if op[0] != "amp":
+        if op[0] not in ("amp", "flush"):
             assert op[1] not in defined
             defined.add(op[1])
+
+
+@pytest.mark.parametrize("n", [2, 3, 4, 5])
+def test_accumulator_blocks_reproduce_term_flows_and_groups_cover_all_terms(n):
+    """Hierarchical JAMP accumulation (plan.py): expanding accumulators through their flush tables gives the
+    same flow x term sign matrix as the direct expansion (also asserted per amplitude inside Plan), and the
+    diagram groups are a partition of the terms that writes every colour flow."""
+    from paper_2312_02898_b200.gen.plan import partition_terms
+    all_terms = topo.diagram_terms(n)
+    groups = partition_terms(n, max_terms=60)
+    assert sorted(map(repr, (t for g in groups for t in g))) == sorted(map(repr, all_terms))
+    fi = topo.flow_index_table(n)
+    direct = {}
+    for t in all_terms:
+        for f, s in topo.term_flows(t, fi):
+            direct[f] = direct.get(f, 0) + abs(s)
+    via = {}
+    for g in groups:
+        p = Plan(n, terms=g)
+        nacc = {}
+        for op in p.ops:
+            if op[0] == "amp":
+                for b, a, s in op[3]:
+                    nacc[(b, a)] = nacc.get((b, a), 0) + 1
+            elif op[0] == "flush":
+                for f, s in op[3]:
+                    via[f] = via.get(f, 0) + abs(s) * nacc[(op[1], op[2])]
+    assert via == direct and set(via) == set(range(len(fi)))
