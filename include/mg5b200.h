@@ -101,7 +101,7 @@ int mg_philox_raw(mg_process_t* p, uint64_t seed, int64_t first_event, int64_t n
  * (MG_FP32).  Asynchronous on `stream`, except that in MG_HEL_FILTER mode the first call runs the
  * helicity probe (K8) on the first min(nevt, 4096) events and synchronises the stream once, and that the
  * processes with >= 24 colour flows keep partial JAMPs in a library-owned workspace (at most MG5B200_WS_GB
- * GiB, default 8; larger batches are processed in event tiles) which is (re)allocated, synchronously, by
+ * GiB, default 16; larger batches are processed in event tiles and helicity chunks) which is (re)allocated, synchronously, by
  * the first call that needs a bigger one. */
 int mg_sigma(mg_process_t* p, const void* momenta_dev, int64_t nevt, void* me_out_dev, void* stream);
 

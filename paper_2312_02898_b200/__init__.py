@@ -13,7 +13,7 @@ import ctypes as C
 import os
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libmg5b200.so")
+LIB_PATH = os.environ.get("MG5B200_LIB") or os.path.join(_HERE, "libmg5b200.so")   # override: kernel experiments
 NEPP = 32
 FP64, FP32 = 0, 1
 HEL_FILTER, HEL_ALL = 0, 1

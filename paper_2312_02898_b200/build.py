@@ -38,6 +38,10 @@ def generate():
             kw["block"] = int(block[str(n)])
         if str(n) in maxterms:
             kw["max_terms"] = int(maxterms[str(n)])
+        if os.environ.get("MG_SYNC"):
+            kw["sync_every"] = int(os.environ["MG_SYNC"])
+        if os.environ.get("MG_MINBLOCKS"):
+            kw["minblocks"] = int(os.environ["MG_MINBLOCKS"])
         jobs.append(emit_ggttng(n, shape=shapes.get(str(n)), **kw))
     keep = set()
     for files, info in jobs:

@@ -37,19 +37,21 @@ struct mg_process {
 };
 
 // Workspace for the split kernel shape: jamp[nhel_run][ncol][2][tile] + meh[nhel_run][tile]; the generated launcher
-// tiles the batch so that it fits.  Capped at MG5B200_WS_GB GiB (default 8).  Grows on demand (synchronous
+// tiles the batch so that it fits.  Capped at MG5B200_WS_GB GiB (default 16).  Grows on demand (synchronous
 // cudaFree/cudaMalloc on the first call that needs more), never shrinks.
 static int ensure_ws(mg_process* p, int64_t nevt, int nhel_run) {
   const int ip = p->par.precision == MG_FP64 ? 0 : 1;
-  const size_t bpe = (size_t)p->desc->ws_bytes_per_event_hel[ip] * (size_t)nhel_run + (size_t)p->desc->ws_bytes_per_event[ip];
-  if (bpe == 0) return MG_OK;
-  double cap_gb = 8.0;
+  const size_t per_eh = (size_t)p->desc->ws_bytes_per_event_hel[ip], per_e = (size_t)p->desc->ws_bytes_per_event[ip];
+  if (per_eh == 0) return MG_OK;
+  double cap_gb = 16.0;
   if (const char* e = getenv("MG5B200_WS_GB")) { const double v = atof(e); if (v > 0) cap_gb = v; }
-  size_t cap = (size_t)(cap_gb * 1073741824.0);
-  if (cap < bpe * 1024) cap = bpe * 1024;
-  const size_t padded = (size_t)((nevt + 31) / 32 * 32);
-  size_t need = padded * bpe;
-  if (need > cap) need = cap / (bpe * 1024) * (bpe * 1024);
+  const size_t cap = (size_t)(cap_gb * 1073741824.0);
+  size_t E = (size_t)((nevt + 31) / 32 * 32);
+  if (E > 131072) E = 131072;
+  size_t need = E * (per_e + (size_t)nhel_run * per_eh);      // whole helicity list resident
+  if (need > cap) need = cap;
+  const size_t floor_bytes = (E < 1024 ? E : 1024) * (per_e + 4 * per_eh);
+  if (need < floor_bytes) need = floor_bytes;
   if (p->ws_bytes >= need) return MG_OK;
   if (p->ws) { cudaDeviceSynchronize(); cudaFree(p->ws); p->ws = nullptr; p->ws_bytes = 0; }
   MG_CUDA(cudaMalloc(&p->ws, need));

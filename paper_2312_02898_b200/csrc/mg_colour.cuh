@@ -51,10 +51,35 @@ __global__ void __launch_bounds__(128) colour_kernel(const double* __restrict__ 
   meh[(long long)ih * stride + ievt] = me;
 }
 
-// fixed-order helicity sum (deterministic), normalisation, optional per-helicity output
+// JAMP[f] = sum of the partial slots the diagram groups wrote for flow f (CSR table ptr/idx), per (event, helicity).
+// Pure streaming: each partial is read once, each JAMP written once; thread = (event, helicity).
+template <class T, int NCOL>
+__global__ void __launch_bounds__(256) gather_kernel(const short* __restrict__ ptr, const short* __restrict__ idx, int npart,
+                                                     const T* __restrict__ part, T* __restrict__ jsum, long long stride,
+                                                     long long nevt) {
+  const long long ievt = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const int ih = blockIdx.y;
+  if (ievt >= nevt) return;
+  const T* __restrict__ pb = part + (long long)ih * npart * 2 * stride + ievt;
+  T* __restrict__ jb = jsum + (long long)ih * (2 * NCOL) * stride + ievt;
+#pragma unroll 4
+  for (int f = 0; f < NCOL; ++f) {
+    T re = T(0), im = T(0);
+    for (int q = ptr[f]; q < ptr[f + 1]; ++q) {
+      const int s = idx[q];
+      re += pb[(2 * s) * stride];
+      im += pb[(2 * s + 1) * stride];
+    }
+    jb[(2 * f) * stride] = re;
+    jb[(2 * f + 1) * stride] = im;
+  }
+}
+
+// fixed-order helicity sum (deterministic), normalisation, optional per-helicity output; `first` = overwrite me_out,
+// else accumulate (helicity chunks are processed one after the other on the same stream)
 template <class T>
 __global__ void helsum_kernel(const T* __restrict__ meh, long long stride, long long nevt, int nhel_run, T norm,
-                              T* __restrict__ me_out, T* __restrict__ perhel_out, long long perhel_stride) {
+                              T* __restrict__ me_out, T* __restrict__ perhel_out, long long perhel_stride, bool first) {
   const long long ievt = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (ievt >= nevt) return;
   T s = T(0);
@@ -63,16 +88,19 @@ __global__ void helsum_kernel(const T* __restrict__ meh, long long stride, long 
     if (perhel_out) perhel_out[(long long)ih * perhel_stride + ievt] = v * norm;
     s += v;
   }
-  me_out[ievt] = s * norm;
+  me_out[ievt] = first ? s * norm : me_out[ievt] + s * norm;
 }
 
 template <class T, int NCOL>
-void colour_and_sum(const double* cft, const T* jamp, T* meh, long long stride, long long nevt, int nhel_run, double norm,
-                    T* me_out, T* perhel_out, long long perhel_stride, cudaStream_t st) {
+void gather_colour_sum(const double* cft, const short* ptr, const short* idx, int npart, const T* part, T* jsum, T* meh,
+                       long long stride, long long nevt, int nhel_run, T norm, T* me_out, T* perhel_out,
+                       long long perhel_stride, bool first, cudaStream_t st) {
+  const dim3 g1((unsigned)((nevt + 255) / 256), (unsigned)nhel_run);
+  gather_kernel<T, NCOL><<<g1, 256, 0, st>>>(ptr, idx, npart, part, jsum, stride, nevt);
   const dim3 grid((unsigned)((nevt + 127) / 128), (unsigned)nhel_run);
-  colour_kernel<T, NCOL><<<grid, 128, 0, st>>>(cft, jamp, meh, stride, nevt, nhel_run);
-  helsum_kernel<T><<<(unsigned)((nevt + 255) / 256), 256, 0, st>>>(meh, stride, nevt, nhel_run, T(norm), me_out, perhel_out,
-                                                                   perhel_stride);
+  colour_kernel<T, NCOL><<<grid, 128, 0, st>>>(cft, jsum, meh, stride, nevt, nhel_run);
+  helsum_kernel<T><<<(unsigned)((nevt + 255) / 256), 256, 0, st>>>(meh, stride, nevt, nhel_run, norm, me_out, perhel_out,
+                                                                   perhel_stride, first);
 }
 
 }  // namespace mgc

@@ -1,0 +1,215 @@
+"""Split kernel shape (n >= 4 gluons): diagram-group kernels + gather + colour + helicity-sum kernels.
+
+Workspace for one tile of E events and one chunk of H helicities (element type T, event index fastest):
+    part[H][NPART][2][E]   partial JAMPs: every diagram group owns a private range of NPART slots (one slot per
+                           colour flow it touches) and writes each exactly once per (event, helicity) — no
+                           read-modify-write, so the group kernels never wait on global loads;
+    jsum[H][NCOL][2][E]    JAMP[f] = sum of the partial slots of flow f (gather kernel, mg_colour.cuh);
+    meh[H][E]              J^dagger CF J per (event, helicity) (colour kernel);
+    inv[NINV][E]           helicity-independent per-event quantities (invariants kernel).
+The launcher loops over event tiles and helicity chunks so that the workspace stays within the size the API
+layer allocated (mg_api.cu: MG5B200_WS_GB).
+"""
+from math import factorial
+
+from .colour import colour_matrix, common_denominator
+from .plan import Plan, partition_terms
+
+
+def emit_split(n, block=128, fp32=True, acc_max=6, max_terms=40, sync_every=2, minblocks=2):
+    from . import emit as E
+    groups = partition_terms(n, max_terms=max_terms)
+    npar, nhel = n + 2, 1 << (n + 2)
+    ns = "mg_ggtt" + "g" * (n - 2)
+    proc = "g g > t t~" + " g" * (n - 2)
+    cf = colour_matrix(n)
+    cfden = common_denominator(cf)
+    ncol = len(cf)
+    cfi = [[int(v * cfden) for v in row] for row in cf]
+    plans = [Plan(n, terms=terms, acc_max=acc_max) for terms in groups]
+    union = E._Union(n, plans)
+    inv = union.items()
+    ninv = union.nitems
+    ndiag = plans[0].ndiagrams
+    files, ginfo = [], []
+    total_flops = 0
+    part_of_flow = {f: [] for f in range(ncol)}     # flow -> global partial slots
+    base = 0
+    for gi, plan in enumerate(plans):
+        flops = plan.flops_per_helicity(colour=False)
+        total_flops += flops
+        touched = sorted(plan.flows_touched())
+        slot = {f: i for i, f in enumerate(touched)}
+        for f in touched:
+            part_of_flow[f].append(base + slot[f])
+        gblock = block
+        while 2 * len(touched) * gblock * 8 > 225 * 1024:
+            gblock -= 32
+        smem64 = 2 * len(touched) * gblock * 8
+        gmin = min(minblocks, 2 if 2 * (smem64 + 1024) <= 227 * 1024 else 1)
+        out = [E.HEADER % dict(proc=proc, n=n, ndiag=ndiag, nterms=len(plan.terms), ncol=ncol, nhel=nhel, flops=flops, ns=ns,
+                               npar=npar, what="diagram group %d of %d (partial JAMP slots %d..%d)"
+                               % (gi, len(plans), base, base + len(touched) - 1))]
+        w = out.append
+        w("constexpr int BLK = %d, NTOUCH = %d, PBASE = %d;\n" % (gblock, len(touched), base))
+        w("template <class T>\n__global__ void __launch_bounds__(%d, %d)\n" % (gblock, gmin))
+        w("group%d_kernel(long long nevt, const int* __restrict__ hel_list, int hcount, int per_thread, int npart,\n"
+          "              T* __restrict__ part, const T* __restrict__ invbuf, long long stride, double mt_d) {\n" % gi)
+        w("  extern __shared__ __align__(16) unsigned char smem_raw[];\n")
+        w("  T* __restrict__ sj = reinterpret_cast<T*>(smem_raw) + threadIdx.x;\n")
+        w("  const long long ievt0 = (long long)blockIdx.x * blockDim.x + threadIdx.x;\n")
+        w("  const bool live = ievt0 < nevt;\n  const long long ievt = live ? ievt0 : nevt - 1;\n")
+        w("  const T* __restrict__ inv = invbuf + ievt;\n  const T mt = T(mt_d);\n")
+        w("  const int ih0 = blockIdx.y * per_thread, ih1 = min(hcount, ih0 + per_thread);\n")
+        w("#pragma unroll 1\n  for (int ih = ih0; ih < ih1; ++ih) {\n")
+        w("    const int h = hel_list[ih];\n")
+        E._externals(plan, w, inv)
+        local_written = set()
+
+        def sink(f, s, re, im, slot=slot, local_written=local_written, w=w):
+            a, b_ = 2 * slot[f], 2 * slot[f] + 1
+            if f in local_written:
+                sg = "+=" if s > 0 else "-="
+                w("    sj[%d * BLK] %s %s; sj[%d * BLK] %s %s;\n" % (a, sg, E._mul(s, re), b_, sg, E._mul(s, im)))
+            else:
+                local_written.add(f)
+                neg = "" if s > 0 else "-"
+                w("    sj[%d * BLK] = %s%s; sj[%d * BLK] = %s%s;\n" % (a, neg, E._mul(s, re), b_, neg, E._mul(s, im)))
+
+        E._body(plan, w, sink, inv, sync_every=sync_every)
+        w("    if (live) {\n")
+        w("      T* __restrict__ pb = part + ((long long)ih * npart + PBASE) * 2 * stride + ievt;\n")
+        w("#pragma unroll\n      for (int q = 0; q < 2 * NTOUCH; ++q) pb[q * stride] = sj[q * BLK];\n")
+        w("    }\n  }\n}\n")
+        w("void launch_group%d(int prec, long long nevt, const int* hel_list, int hcount, int per_thread, int npart, void* part,\n"
+          "                    const void* inv, long long stride, double mt, cudaStream_t st) {\n" % gi)
+        w("  const dim3 grid((unsigned)((nevt + BLK - 1) / BLK), (unsigned)((hcount + per_thread - 1) / per_thread));\n")
+        w("  static bool attr_set = false;\n  if (!attr_set) {\n")
+        w("    cudaFuncSetAttribute(group%d_kernel<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * NTOUCH * BLK * 8);\n" % gi)
+        if fp32:
+            w("    cudaFuncSetAttribute(group%d_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * NTOUCH * BLK * 4);\n" % gi)
+        w("    attr_set = true;\n  }\n")
+        w("  if (prec == 0) group%d_kernel<double><<<grid, BLK, 2 * NTOUCH * BLK * 8, st>>>(nevt, hel_list, hcount, per_thread, npart, (double*)part, (const double*)inv, stride, mt);\n" % gi)
+        if fp32:
+            w("  else group%d_kernel<float><<<grid, BLK, 2 * NTOUCH * BLK * 4, st>>>(nevt, hel_list, hcount, per_thread, npart, (float*)part, (const float*)inv, stride, mt);\n" % gi)
+        w("}\n}  // namespace\n")
+        files.append(("%s_g%02d.cu" % (ns, gi), "".join(out)))
+        ginfo.append(dict(terms=len(plan.terms), counts=plan.counts(), max_live=plan.max_live(), flops=flops,
+                          flows=len(touched), block=gblock, minblocks=gmin, smem64=smem64))
+        base += len(touched)
+    npart = base
+    assert all(part_of_flow[f] for f in range(ncol)), "every colour flow must be written by some group"
+    files.append(_main_unit(E, n, ns, proc, npar, nhel, ncol, ndiag, cfi, cfden, union, inv, ninv, npart, part_of_flow,
+                            len(plans), total_flops, fp32))
+    colour_flops = 2 * (ncol * (ncol - 1) // 2) * 2 + ncol * 8
+    info = dict(proc=proc, ns=ns, npar=npar, ncol=ncol, nhel=nhel, ndiagrams=ndiag, nterms=sum(len(g) for g in groups),
+                flops_per_helicity=total_flops + colour_flops, shape="split", ngroups=len(plans), npart=npart, ninv=ninv,
+                groups=ginfo)
+    return files, info
+
+
+def _main_unit(E, n, ns, proc, npar, nhel, ncol, ndiag, cfi, cfden, union, inv, ninv, npart, part_of_flow, ngroups,
+               group_flops, fp32):
+    colour_flops = 2 * (ncol * (ncol - 1) // 2) * 2 + ncol * 8
+    denom = 4 * 64 * factorial(n - 2)
+    rows = E._colour_rows(cfi, ncol)
+    out = [E.HEADER % dict(proc=proc, n=n, ndiag=ndiag, nterms=0, ncol=ncol, nhel=nhel, flops=colour_flops, ns=ns, npar=npar,
+                           what="invariants kernel, JAMP gather, colour sum (K6), helicity sum (K7), tile loop over the "
+                                "%d diagram-group kernels" % ngroups)]
+    w = out.append
+    w('#include "mg_colour.cuh"\n')
+    w("// symmetric colour form: me = sum_i J_i^* (CF_ii J_i + 2 sum_{j>i} CF_ij J_j) / %d ; rows blocked by 8\n" % cfden)
+    tab = []
+    for i0 in range(0, ncol, 8):
+        for j in range(i0, ncol):
+            for i in range(i0, i0 + 8):
+                tab.append(rows[i][j] if i < ncol else 0)
+    w("__device__ __align__(16) const double cf_table[%d] = {\n" % len(tab))
+    for k_ in range(0, len(tab), 24):
+        w("  " + ", ".join("%d." % v for v in tab[k_:k_ + 24]) + ",\n")
+    w("};\n")
+    # gather table (CSR): flow f <- partial slots part_idx[part_ptr[f] .. part_ptr[f+1])
+    ptr, idx = [0], []
+    for f in range(ncol):
+        idx += part_of_flow[f]
+        ptr.append(len(idx))
+    w("constexpr int NPART = %d, NINV = %d;\n" % (npart, ninv))
+    w("__device__ const short part_ptr[%d] = {%s};\n" % (len(ptr), ", ".join(map(str, ptr))))
+    w("__device__ const short part_idx[%d] = {\n" % len(idx))
+    for k_ in range(0, len(idx), 32):
+        w("  " + ", ".join(map(str, idx[k_:k_ + 32])) + ",\n")
+    w("};\n")
+    for gi in range(ngroups):
+        w("void launch_group%d(int prec, long long nevt, const int* hel_list, int hcount, int per_thread, int npart, void* part,\n"
+          "                    const void* inv, long long stride, double mt, cudaStream_t st);\n" % gi)
+    w("template <class T>\n__global__ void __launch_bounds__(128) invariants_kernel(const double* __restrict__ mom, long long nevt,\n"
+      "                  T* __restrict__ invbuf, long long stride, double mt_d) {\n")
+    w("  const long long ievt = (long long)blockIdx.x * blockDim.x + threadIdx.x;\n  if (ievt >= nevt) return;\n")
+    E._prologue(union, w)
+    w("  T* __restrict__ o = invbuf + ievt;\n")
+    for name, i in sorted(inv.items(), key=lambda kv: kv[1]):
+        if name[0] == "s":
+            w("  o[%d * stride] = %s;\n" % (i, name))
+        else:
+            src = "k[%s]" % name[1:] if name[0] == "k" else name
+            w("  stp(o + %d * stride, stride, %s);\n" % (i, src))
+    w("}\n")
+    w("""
+template <class T>
+static void run(const double* mom, T* me_out, long long nevt, const int* hel_list, int nhel_run, T* perhel_out,
+                const double* par, void* ws, size_t ws_bytes, cudaStream_t st, int prec) {
+  double norm = 1.0;
+  for (int i = 0; i < NGLU; ++i) norm *= par[0];          // par[0] = g_s^2, par[1] = mt
+  norm /= (double)%(cfden)d * (double)%(denom)d;
+  const size_t es = sizeof(T);
+  const size_t per_eh = (size_t)(2 * NPART + 2 * NCOL + 1) * es;     // bytes per (event, helicity)
+  const size_t per_e = (size_t)NINV * es;                            // bytes per event
+  // event tile E (multiple of 1024, or the whole padded batch) and helicity chunk H
+  long long E = (nevt + 31) / 32 * 32;
+  if (E > 131072) E = 131072;
+  while (E > 1024 && (size_t)E * (per_e + 4 * per_eh) > ws_bytes) E = (E / 2 + 1023) / 1024 * 1024;
+  if ((size_t)E * (per_e + per_eh) > ws_bytes) return;              // mg_api.cu sizes the workspace; cannot happen
+  long long H = (long long)((ws_bytes / (size_t)E - per_e) / per_eh);
+  if (H > nhel_run) H = nhel_run;
+  const double* cft = nullptr; const short* pptr = nullptr; const short* pidx = nullptr;
+  cudaGetSymbolAddress((void**)&cft, cf_table);
+  cudaGetSymbolAddress((void**)&pptr, part_ptr);
+  cudaGetSymbolAddress((void**)&pidx, part_idx);
+  T* part = (T*)ws;
+  T* jsum = part + (size_t)H * 2 * NPART * E;
+  T* meh = jsum + (size_t)H * 2 * NCOL * E;
+  T* inv = meh + (size_t)H * E;
+  for (long long e0 = 0; e0 < nevt; e0 += E) {
+    const long long ne = nevt - e0 < E ? nevt - e0 : E;
+    const double* m0 = mom + e0 * NPAR * 4;       // tile starts on a page boundary
+    invariants_kernel<T><<<(unsigned)((ne + 127) / 128), 128, 0, st>>>(m0, ne, inv, E, par[1]);
+    for (int h0 = 0; h0 < nhel_run; h0 += (int)H) {
+      const int hc = nhel_run - h0 < H ? nhel_run - h0 : (int)H;
+      // helicities per thread: keep >= ~4 waves of threads in flight
+      long long slices = (148LL * 256 * 4 + ne - 1) / ne;
+      if (slices > hc) slices = hc;
+      if (slices < 1) slices = 1;
+      const int per_thread = (int)((hc + slices - 1) / slices);
+%(calls)s
+      mgc::gather_colour_sum<T, NCOL>(cft, pptr, pidx, NPART, part, jsum, meh, E, ne, hc, T(norm), me_out + e0,
+                                      perhel_out ? perhel_out + (long long)h0 * nevt + e0 : (T*)nullptr, nevt, h0 == 0, st);
+    }
+  }
+}
+static void launch(int prec, const double* mom, void* me_out, long long nevt, const int* hel_list, int nhel_run,
+                   void* perhel_out, const double* par, void* ws, size_t ws_bytes, cudaStream_t st) {
+  if (prec == 0) run<double>(mom, (double*)me_out, nevt, hel_list, nhel_run, (double*)perhel_out, par, ws, ws_bytes, st, prec);
+%(run32)s
+}
+}  // namespace
+extern const mg_procdesc_t mg_desc_%(tag)s = {"%(proc)s", %(npar)d, %(nfinal)d, %(ndiag)d, %(nhel)d, %(ncol)d, %(denom)d,
+  %(flops)dLL, {0, 0, 1, 1%(gm)s}, %(ns)s::launch, {%(ws64)d, %(ws32)d}, %(nk)d, %(hasfp32)d, {%(wse64)d, %(wse32)d}};
+""" % dict(cfden=cfden, denom=denom, tag=ns[3:], proc=proc, npar=npar, nfinal=n, ndiag=ndiag, nhel=nhel, ncol=ncol,
+           flops=group_flops + colour_flops, gm=", 0" * (n - 2), ns=ns,
+           ws64=(2 * npart + 2 * ncol + 1) * 8, ws32=(2 * npart + 2 * ncol + 1) * 4,
+           nk=ngroups + 4, hasfp32=1 if fp32 else 0, wse64=ninv * 8, wse32=ninv * 4,
+           calls="\n".join("      launch_group%d(prec, ne, hel_list + h0, hc, per_thread, NPART, part, inv, E, par[1], st);" % gi
+                           for gi in range(ngroups)),
+           run32=("  else run<float>(mom, (float*)me_out, nevt, hel_list, nhel_run, (float*)perhel_out, par, ws, ws_bytes, st, prec);"
+                  if fp32 else "")))
+    return (ns + ".cu", "".join(out))

@@ -320,7 +320,13 @@ def group_key(term, n):
     anc = anchor_of(mid, th)
     la = topo.leaves_of(anc)
     if th <= len(la) < n:
-        return ("A", tuple(sorted(la)))
+        # sub-key: the (|anchor|-1)-gluon sub-tree the anchor is built on, if it is v3(sub-tree, leaf)
+        sub = "x"
+        if n >= 5 and anc[0] == "v3":
+            for big, small in ((anc[1], anc[2]), (anc[2], anc[1])):
+                if small[0] == "g" and len(topo.leaves_of(big)) == len(la) - 1:
+                    sub = tuple(sorted(topo.leaves_of(big)))
+        return ("A", tuple(sorted(la)), sub)
     if len(la) >= n:
         return ("T", mid[0])
     if c > 0:
