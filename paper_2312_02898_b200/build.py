@@ -38,6 +38,8 @@ def generate():
             kw["block"] = int(block[str(n)])
         if str(n) in maxterms:
             kw["max_terms"] = int(maxterms[str(n)])
+        if os.environ.get("MG_LIVEMAX"):
+            kw["live_max"] = int(os.environ["MG_LIVEMAX"])
         if os.environ.get("MG_SYNC"):
             kw["sync_every"] = int(os.environ["MG_SYNC"])
         if os.environ.get("MG_MINBLOCKS"):

@@ -16,9 +16,41 @@ from .colour import colour_matrix, common_denominator
 from .plan import Plan, partition_terms
 
 
-def emit_split(n, block=128, fp32=True, acc_max=6, max_terms=40, sync_every=2, minblocks=2):
+def choose_kernels(n, max_terms, live_max, acc_max, flat_phase=0):
+    """Kernels (coarse diagram groups) and their phases: every kernel is split into as few phases as keep the
+    number of simultaneously live currents of each phase <= live_max (register pressure), because every extra
+    phase recomputes the low-multiplicity currents it shares with its neighbours."""
+    import os
+    flat = int(os.environ.get("MG_FLATPHASE", "0")) or flat_phase
+    if flat:
+        # every phase its own kernel: short straight-line bodies that stay resident in the instruction caches
+        return [[Plan(n, terms=ph, acc_max=acc_max)] for k in partition_terms(n, max_terms=max_terms, max_phase=flat)
+                for ph in k]
+    cands = [10 ** 6, 128, 96, 64, 48, 32, 24, 16, 8]
+    parts = {mp: partition_terms(n, max_terms=max_terms, max_phase=mp) for mp in cands}
+    out = []
+    for i in range(len(parts[cands[0]])):
+        for mp in cands:
+            plans = [Plan(n, terms=ph, acc_max=acc_max) for ph in parts[mp][i]]
+            if max(p.max_live() for p in plans) <= live_max or mp == cands[-1]:
+                out.append(plans)
+                break
+    return out
+
+
+# measured on B200 (DESIGN.md §7): short kernels win — their straight-line bodies stay in the instruction caches and
+# their live state fits the register file — even though every extra kernel recomputes a few shared currents and
+# adds partial-JAMP slots.  n = 4: 8 kernels of <= 40 terms; n = 5: 63 kernels of <= 32 terms.
+TUNED = {4: dict(max_terms=40, live_max=1000, flat_phase=0), 5: dict(max_terms=170, live_max=12, flat_phase=32)}
+
+
+def emit_split(n, block=128, fp32=True, acc_max=6, max_terms=None, sync_every=2, minblocks=2, live_max=None, flat_phase=None):
     from . import emit as E
-    groups = partition_terms(n, max_terms=max_terms)
+    tuned = TUNED.get(n, TUNED[5])
+    max_terms = max_terms or tuned["max_terms"]
+    live_max = live_max or tuned["live_max"]
+    flat_phase = tuned["flat_phase"] if flat_phase is None else flat_phase
+    kernels = choose_kernels(n, max_terms, live_max, acc_max, flat_phase)
     npar, nhel = n + 2, 1 << (n + 2)
     ns = "mg_ggtt" + "g" * (n - 2)
     proc = "g g > t t~" + " g" * (n - 2)
@@ -26,7 +58,7 @@ def emit_split(n, block=128, fp32=True, acc_max=6, max_terms=40, sync_every=2, m
     cfden = common_denominator(cf)
     ncol = len(cf)
     cfi = [[int(v * cfden) for v in row] for row in cf]
-    plans = [Plan(n, terms=terms, acc_max=acc_max) for terms in groups]
+    plans = [p for k in kernels for p in k]
     union = E._Union(n, plans)
     inv = union.items()
     ninv = union.nitems
@@ -35,10 +67,14 @@ def emit_split(n, block=128, fp32=True, acc_max=6, max_terms=40, sync_every=2, m
     total_flops = 0
     part_of_flow = {f: [] for f in range(ncol)}     # flow -> global partial slots
     base = 0
-    for gi, plan in enumerate(plans):
-        flops = plan.flops_per_helicity(colour=False)
+    nkern = len(kernels)
+    ext_flops = Plan(n, terms=[]).flops_per_helicity(colour=False)      # external wavefunctions, once per kernel
+    for gi, phases in enumerate(kernels):
+        flops = sum(p.flops_per_helicity(colour=False, externals=False) for p in phases) + ext_flops
         total_flops += flops
-        touched = sorted(plan.flows_touched())
+        touched = sorted(set().union(*[p.flows_touched() for p in phases]))
+        nterms = sum(len(p.terms) for p in phases)
+        live = max(p.max_live() for p in phases)
         slot = {f: i for i, f in enumerate(touched)}
         for f in touched:
             part_of_flow[f].append(base + slot[f])
@@ -47,9 +83,9 @@ def emit_split(n, block=128, fp32=True, acc_max=6, max_terms=40, sync_every=2, m
             gblock -= 32
         smem64 = 2 * len(touched) * gblock * 8
         gmin = min(minblocks, 2 if 2 * (smem64 + 1024) <= 227 * 1024 else 1)
-        out = [E.HEADER % dict(proc=proc, n=n, ndiag=ndiag, nterms=len(plan.terms), ncol=ncol, nhel=nhel, flops=flops, ns=ns,
-                               npar=npar, what="diagram group %d of %d (partial JAMP slots %d..%d)"
-                               % (gi, len(plans), base, base + len(touched) - 1))]
+        out = [E.HEADER % dict(proc=proc, n=n, ndiag=ndiag, nterms=nterms, ncol=ncol, nhel=nhel, flops=flops, ns=ns,
+                               npar=npar, what="diagram group %d of %d, %d phase(s) (partial JAMP slots %d..%d)"
+                               % (gi, nkern, len(phases), base, base + len(touched) - 1))]
         w = out.append
         w("constexpr int BLK = %d, NTOUCH = %d, PBASE = %d;\n" % (gblock, len(touched), base))
         w("template <class T>\n__global__ void __launch_bounds__(%d, %d)\n" % (gblock, gmin))
@@ -63,7 +99,7 @@ def emit_split(n, block=128, fp32=True, acc_max=6, max_terms=40, sync_every=2, m
         w("  const int ih0 = blockIdx.y * per_thread, ih1 = min(hcount, ih0 + per_thread);\n")
         w("#pragma unroll 1\n  for (int ih = ih0; ih < ih1; ++ih) {\n")
         w("    const int h = hel_list[ih];\n")
-        E._externals(plan, w, inv)
+        E._externals(_AllExternals(n), w, inv)
         local_written = set()
 
         def sink(f, s, re, im, slot=slot, local_written=local_written, w=w):
@@ -76,7 +112,10 @@ def emit_split(n, block=128, fp32=True, acc_max=6, max_terms=40, sync_every=2, m
                 neg = "" if s > 0 else "-"
                 w("    sj[%d * BLK] = %s%s; sj[%d * BLK] = %s%s;\n" % (a, neg, E._mul(s, re), b_, neg, E._mul(s, im)))
 
-        E._body(plan, w, sink, inv, sync_every=sync_every)
+        for pi, plan in enumerate(phases):
+            w("    {   // phase %d: %d terms, <= %d live currents\n" % (pi, len(plan.terms), plan.max_live()))
+            E._body(plan, w, sink, inv, sync_every=sync_every)
+            w("    }\n")
         w("    if (live) {\n")
         w("      T* __restrict__ pb = part + ((long long)ih * npart + PBASE) * 2 * stride + ievt;\n")
         w("#pragma unroll\n      for (int q = 0; q < 2 * NTOUCH; ++q) pb[q * stride] = sj[q * BLK];\n")
@@ -94,18 +133,26 @@ def emit_split(n, block=128, fp32=True, acc_max=6, max_terms=40, sync_every=2, m
             w("  else group%d_kernel<float><<<grid, BLK, 2 * NTOUCH * BLK * 4, st>>>(nevt, hel_list, hcount, per_thread, npart, (float*)part, (const float*)inv, stride, mt);\n" % gi)
         w("}\n}  // namespace\n")
         files.append(("%s_g%02d.cu" % (ns, gi), "".join(out)))
-        ginfo.append(dict(terms=len(plan.terms), counts=plan.counts(), max_live=plan.max_live(), flops=flops,
+        ginfo.append(dict(terms=nterms, phases=[len(p.terms) for p in phases], max_live=live, flops=flops,
                           flows=len(touched), block=gblock, minblocks=gmin, smem64=smem64))
         base += len(touched)
     npart = base
     assert all(part_of_flow[f] for f in range(ncol)), "every colour flow must be written by some group"
     files.append(_main_unit(E, n, ns, proc, npar, nhel, ncol, ndiag, cfi, cfden, union, inv, ninv, npart, part_of_flow,
-                            len(plans), total_flops, fp32))
+                            nkern, total_flops, fp32))
     colour_flops = 2 * (ncol * (ncol - 1) // 2) * 2 + ncol * 8
-    info = dict(proc=proc, ns=ns, npar=npar, ncol=ncol, nhel=nhel, ndiagrams=ndiag, nterms=sum(len(g) for g in groups),
-                flops_per_helicity=total_flops + colour_flops, shape="split", ngroups=len(plans), npart=npart, ninv=ninv,
+    info = dict(proc=proc, ns=ns, npar=npar, ncol=ncol, nhel=nhel, ndiagrams=ndiag, nterms=sum(len(p.terms) for p in plans),
+                flops_per_helicity=total_flops + colour_flops, shape="split", ngroups=nkern, npart=npart, ninv=ninv,
                 groups=ginfo)
     return files, info
+
+
+class _AllExternals:
+    """Stand-in plan for _externals(): every external wavefunction is used somewhere in a multi-phase kernel."""
+
+    def __init__(self, n):
+        self.n = n
+        self.ops = [("x",) + tuple("e%d" % i for i in range(n))]
 
 
 def _main_unit(E, n, ns, proc, npar, nhel, ncol, ndiag, cfi, cfden, union, inv, ninv, npart, part_of_flow, ngroups,

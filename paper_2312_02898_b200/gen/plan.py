@@ -30,6 +30,7 @@ The plan is a flat list of ops in evaluation order:
    ("flush", block, a, flows)           JAMP[f] += sign*acc[block][a] for (f, sign) in flows
 Names: external gluons "e<i>", "ub" (ubar(p_t)), "vv" (v(p_t~)); internal "w<k>".
 """
+import os
 from math import factorial
 
 from . import topology as topo
@@ -92,7 +93,7 @@ def skeleton_key(skel, frontier):
 class Plan:
     """Ops for an ordered list of terms (default: all terms of the process, sorted for locality)."""
 
-    def __init__(self, n, terms=None, acc_max=6, sort=True):
+    def __init__(self, n, terms=None, acc_max=6, sort=True, max_keep=0):
         self.n = n
         self.flow_index = topo.flow_index_table(n)
         self.ncol = len(self.flow_index)
@@ -101,10 +102,12 @@ class Plan:
         self.terms = list(all_terms if terms is None else terms)
         self.acc_max = acc_max
         self.ops = []
-        self._g = {}
-        self._l = {(): "ub"}
-        self._r = {(): "vv"}
-        self._b = {}
+        # memo of internal currents, least recently used first.  max_keep > 0 bounds it: a current that has not
+        # been used for a while is dropped and *recomputed* if it is needed again (rematerialisation), which keeps
+        # the number of simultaneously live currents — registers — bounded at the price of a few extra FLOPs.
+        from collections import OrderedDict
+        self._memo = OrderedDict()
+        self.max_keep = max_keep
         self._next = 0
         self.gmasks = set()      # gluon-propagator subsets
         self.lmasks = set()      # top-side quark propagators
@@ -117,11 +120,25 @@ class Plan:
         return "w%d" % (self._next - 1)
 
     # ---- currents ----
+    def _get(self, key):
+        if key in self._memo:
+            self._memo.move_to_end(key)
+            return self._memo[key]
+        return None
+
+    def _put(self, key, name):
+        self._memo[key] = name
+        if self.max_keep:
+            while len(self._memo) > self.max_keep:
+                self._memo.popitem(last=False)
+        return name
+
     def g(self, tree):
         if tree[0] == "g":
             return "e%d" % tree[1]
-        if tree in self._g:
-            return self._g[tree]
+        hit = self._get(("g", tree))
+        if hit:
+            return hit
         mask = topo.leafmask(tree)
         self.gmasks.add(mask)
         if tree[0] == "v3":
@@ -132,12 +149,14 @@ class Plan:
             a, m, c = self.g(tree[1]), self.g(tree[2]), self.g(tree[3])
             out = self._new()
             self.ops.append(("k", out, a, m, c, mask))
-        self._g[tree] = out
-        return out
+        return self._put(("g", tree), out)
 
     def l(self, chain):
-        if chain in self._l:
-            return self._l[chain]
+        if not chain:
+            return "ub"
+        hit = self._get(("l", chain))
+        if hit:
+            return hit
         prev = self.l(chain[:-1])
         gc = self.g(chain[-1])
         mask = 0
@@ -146,12 +165,14 @@ class Plan:
         self.lmasks.add(mask)
         out = self._new()
         self.ops.append(("lq", out, prev, gc, mask))
-        self._l[chain] = out
-        return out
+        return self._put(("l", chain), out)
 
     def r(self, chain):
-        if chain in self._r:
-            return self._r[chain]
+        if not chain:
+            return "vv"
+        hit = self._get(("r", chain))
+        if hit:
+            return hit
         nxt = self.r(chain[1:])
         gc = self.g(chain[0])
         mask = 0
@@ -160,16 +181,16 @@ class Plan:
         self.rmasks.add(mask)
         out = self._new()
         self.ops.append(("rq", out, nxt, gc, mask))
-        self._r[chain] = out
-        return out
+        return self._put(("r", chain), out)
 
-    def b(self, lname, rname):
-        key = (lname, rname)
-        if key not in self._b:
-            out = self._new()
-            self.ops.append(("bil", out, lname, rname))
-            self._b[key] = out
-        return self._b[key]
+    def b(self, lchain, rchain):
+        hit = self._get(("b", lchain, rchain))
+        if hit:
+            return hit
+        ln, rn = self.l(lchain), self.r(rchain)
+        out = self._new()
+        self.ops.append(("bil", out, ln, rn))
+        return self._put(("b", lchain, rchain), out)
 
     # ---- accumulation blocks ----
     def _block(self, lchain, rchain, mid):
@@ -224,12 +245,12 @@ class Plan:
             keyed.append((term[:c], term[c + 1:], term[c], term))
         if sort:
             keyed.sort(key=lambda k: amp_sort_key(k[0], k[1], k[2], self.acc_max, self.n))
+            if os.environ.get("MG_GREEDY", "1") == "1":
+                keyed = _greedy_order(keyed, self.acc_max)
         self.namps = 0
         open_blocks = []
         for lchain, rchain, mid, term in keyed:
-            ln = self.l(lchain)
-            rn = self.r(rchain)
-            bn = self.b(ln, rn)
+            bn = self.b(lchain, rchain)
             gn = self.g(mid)
             blk, accs = self._block(lchain, rchain, mid)
             # consistency: expanding the accumulators reproduces the term's flow list exactly
@@ -286,20 +307,128 @@ class Plan:
         return s
 
     def max_live(self):
-        """Peak number of simultaneously live internal currents in program order (register-pressure proxy)."""
+        """Peak live state in program order, in units of one current (8 doubles): internal currents plus open
+        JAMP accumulators (a quarter each) — the register-pressure proxy the phase splitting is steered by."""
         last = {}
         for i, op in enumerate(self.ops):
             for nm in _inputs(op):
                 last[nm] = i
-        live, peak = set(), 0
+        acc_last = {}
+        for i, op in enumerate(self.ops):
+            if op[0] == "flush":
+                acc_last[(op[1], op[2])] = i
+        live, accs, peak = set(), set(), 0.0
         for i, op in enumerate(self.ops):
             if op[0] not in ("amp", "flush"):
                 live.add(op[1])
-            peak = max(peak, len(live))
+            if op[0] == "amp":
+                accs.update((b_, a) for b_, a, _ in op[3])
+            peak = max(peak, len(live) + 0.25 * len(accs))
             for nm in _inputs(op):
                 if last.get(nm) == i and nm in live:
                     live.discard(nm)
-        return peak
+            if op[0] == "flush" and acc_last.get((op[1], op[2])) == i:
+                accs.discard((op[1], op[2]))
+        return int(peak + 0.75)
+
+
+# ------------------------------------------------------------------------------------------ amplitude order
+def _deps(key):
+    """Direct inputs (as memo keys) of an internal current; external wavefunctions are not listed."""
+    kind = key[0]
+    if kind == "g":
+        return [("g", c) for c in key[1][1:] if c[0] != "g"]
+    if kind == "l":
+        chain = key[1]
+        return ([("l", chain[:-1])] if len(chain) > 1 else []) + ([("g", chain[-1])] if chain[-1][0] != "g" else [])
+    if kind == "r":
+        chain = key[1]
+        return ([("r", chain[1:])] if len(chain) > 1 else []) + ([("g", chain[0])] if chain[0][0] != "g" else [])
+    if kind == "b":
+        return ([("l", key[1])] if key[1] else []) + ([("r", key[2])] if key[2] else [])
+    raise AssertionError(kind)
+
+
+def _amp_accs(mid, acc_max):
+    """(skeleton key, accumulator ids) of the amplitude of a mid tree: see Plan._block."""
+    from itertools import product
+    skel, frontier = skeleton(mid, acc_max)
+    combos = [tuple(c[0] for c in choice) for choice in product(*[topo.orderings(f) for f in frontier])]
+    return skeleton_key(skel, frontier), combos
+
+
+def _greedy_order(keyed, acc_max):
+    """Register-pressure-aware order of the amplitudes (list scheduling on the current DAG): repeatedly take the
+    amplitude that adds the least live state — not-yet-computed currents (8 doubles each) and newly opened JAMP
+    accumulators (2 doubles each) — net of what it lets die (currents whose consumers are all done, accumulator
+    blocks whose last amplitude this is); ties keep the locality order given.  No current is computed twice."""
+    namp = len(keyed)
+    roots, closure, blocks, accs = [], [], [], []
+    consumers = {}           # current key -> number of direct consumers (currents or amplitudes) still to come
+    block_left = {}          # block key -> amplitudes still to come
+    seen_nodes = set()
+    for lchain, rchain, mid, term in keyed:
+        r_ = [("b", lchain, rchain)] + ([("g", mid)] if mid[0] != "g" else [])
+        roots.append(r_)
+        clo, stack = [], list(r_)
+        while stack:
+            k = stack.pop()
+            if k in clo:
+                continue
+            clo.append(k)
+            stack.extend(_deps(k))
+        closure.append(clo)
+        sk, combos = _amp_accs(mid, acc_max)
+        bkey = (lchain, rchain, sk)
+        blocks.append(bkey)
+        accs.append([(bkey, c) for c in combos])
+        block_left[bkey] = block_left.get(bkey, 0) + 1
+        for k in r_:
+            consumers[k] = consumers.get(k, 0) + 1
+        for k in clo:
+            if k not in seen_nodes:
+                seen_nodes.add(k)
+                for d in _deps(k):
+                    consumers[d] = consumers.get(d, 0) + 1
+    computed = set()
+    open_accs = {}           # block key -> set of open accumulator ids
+    remaining = list(range(namp))
+    order = []
+    while remaining:
+        best, best_score = None, None
+        for pos, i in enumerate(remaining):
+            new = [k for k in closure[i] if k not in computed]
+            dec = {}
+            for k in new:
+                for d in _deps(k):
+                    dec[d] = dec.get(d, 0) + 1
+            for k in roots[i]:
+                dec[k] = dec.get(k, 0) + 1
+            freed = sum(1 for k, v in dec.items() if consumers[k] - v == 0)
+            opened = open_accs.get(blocks[i], ())
+            new_acc = sum(1 for a in accs[i] if a not in opened)
+            freed_acc = (len(opened) + new_acc) if block_left[blocks[i]] == 1 else 0
+            score = (8 * (len(new) - freed) + 2 * (new_acc - freed_acc), len(new), pos)
+            if best_score is None or score < best_score:
+                best, best_score = i, score
+            if score[0] < 0 or (score[0] == 0 and score[1] == 0):
+                break           # shrinks (or keeps) the live set right away: take it
+        i = best
+        for k in closure[i]:
+            if k not in computed:
+                computed.add(k)
+                for d in _deps(k):
+                    consumers[d] -= 1
+        for k in roots[i]:
+            consumers[k] -= 1
+        block_left[blocks[i]] -= 1
+        if block_left[blocks[i]] == 0:
+            open_accs.pop(blocks[i], None)
+        else:
+            open_accs.setdefault(blocks[i], set()).update(accs[i])
+        order.append(keyed[i])
+        remaining.remove(i)
+    return order
 
 
 def anchor_of(mid, th=4):
@@ -313,30 +442,37 @@ def anchor_of(mid, th=4):
 
 
 def group_key(term, n):
-    """Locality key of a term: terms with the same key share their expensive currents."""
+    """(coarse, fine) locality key of a term.  Terms with the same coarse key go into the same kernel (they feed
+    the same few colour flows); terms with the same fine key share their expensive currents and form a *phase*
+    (its own Plan: the few low-multiplicity currents it shares with other phases are recomputed, so that very
+    little is live across phases)."""
     th = max(n - 1, 2)
     c = closure_block(term)
     mid = term[c]
     anc = anchor_of(mid, th)
     la = topo.leaves_of(anc)
+
+    def big_child(t):
+        if t[0] == "g":
+            return ()
+        kids = sorted(t[1:], key=lambda k: -len(topo.leaves_of(k)))
+        return tuple(sorted(topo.leaves_of(kids[0])))
+
     if th <= len(la) < n:
-        # sub-key: the (|anchor|-1)-gluon sub-tree the anchor is built on, if it is v3(sub-tree, leaf)
-        sub = "x"
-        if n >= 5 and anc[0] == "v3":
-            for big, small in ((anc[1], anc[2]), (anc[2], anc[1])):
-                if small[0] == "g" and len(topo.leaves_of(big)) == len(la) - 1:
-                    sub = tuple(sorted(topo.leaves_of(big)))
-        return ("A", tuple(sorted(la)), sub)
+        return ("A", tuple(sorted(la))), big_child(anc)
     if len(la) >= n:
-        return ("T", mid[0])
+        return ("T", mid[0]), big_child(mid)
     if c > 0:
-        return ("L", tuple(sorted(topo.leaves_of(term[0]))))
-    return ("R", tuple(sorted(topo.leaves_of(term[-1]))))
+        nxt = tuple(sorted(topo.leaves_of(term[1])))
+        return ("L", tuple(sorted(topo.leaves_of(term[0])))), nxt
+    prv = tuple(sorted(topo.leaves_of(term[-2]))) if len(term) > 1 else ()
+    return ("R", tuple(sorted(topo.leaves_of(term[-1])))), prv
 
 
 def amp_sort_key(lchain, rchain, mid, acc_max, n):
     term = lchain + (mid,) + rchain
     gk = group_key(term, n)
+    gk = (gk[0][0], gk[0][1], gk[1])
     anc = anchor_of(mid, max(n - 1, 2))
     skel, frontier = skeleton(anc, acc_max)
     big = gk[0] in ("A", "T")
@@ -360,33 +496,41 @@ def _inputs(op):
 
 
 # ------------------------------------------------------------------------------------------ diagram groups
-def partition_terms(n, max_terms=170):
-    """Splits the terms of g g -> t t~ + (n-2) g into diagram groups (one kernel each).
-    Terms anchored on a >= 4-gluon sub-tree go with that sub-tree's leaf set (its current is computed once and
-    used by every amplitude that contains it); the rest are keyed by the outermost quark-line block they share
-    and bin-packed."""
+def partition_terms(n, max_terms=170, max_phase=32):
+    """Splits the terms of g g -> t t~ + (n-2) g into kernels and phases: returns a list of kernels, each a list
+    of phases, each a list of terms.  Coarse keys (group_key) make kernels — small ones are bin-packed up to
+    `max_terms` —, fine keys make phases, bin-packed up to `max_phase` terms."""
     terms = topo.diagram_terms(n)
-    buckets = {}
+    coarse = {}
     for term in terms:
-        buckets.setdefault(group_key(term, n), []).append(term)
-    total = len(terms)
-    if total <= max_terms:
-        return [terms]
-    groups = []
-    small = []
-    for key in sorted(buckets, key=lambda k: (k[0], k[1])):
-        b = buckets[key]
-        if key[0] in ("A", "T"):
-            groups.append(b)
-        else:
-            small.append(b)
-    cur = []
-    for b in small:
-        if cur and len(cur) + len(b) > max_terms:
-            groups.append(cur)
-            cur = []
-        cur = cur + b
+        ck, fk = group_key(term, n)
+        coarse.setdefault(ck, {}).setdefault(fk, []).append(term)
+
+    def phases_of(fine):
+        out, cur = [], []
+        for fk in sorted(fine, key=repr):
+            b = fine[fk]
+            if cur and len(cur) + len(b) > max_phase:
+                out.append(cur)
+                cur = []
+            cur = cur + b
+        if cur:
+            out.append(cur)
+        return out
+
+    kernels, cur, cur_n = [], {}, 0
+    for ck in sorted(coarse, key=repr):
+        fine = {(ck, fk): v for fk, v in coarse[ck].items()}
+        nt = sum(len(v) for v in fine.values())
+        if ck[0] in ("A", "T") or nt >= max_terms:
+            kernels.append(phases_of(fine))
+            continue
+        if cur and cur_n + nt > max_terms:
+            kernels.append(phases_of(cur))
+            cur, cur_n = {}, 0
+        cur.update(fine)
+        cur_n += nt
     if cur:
-        groups.append(cur)
-    assert sum(len(g) for g in groups) == total
-    return groups
+        kernels.append(phases_of(cur))
+    assert sum(len(p) for k in kernels for p in k) == len(terms)
+    return kernels

@@ -90,7 +90,8 @@ def test_accumulator_blocks_reproduce_term_flows_and_groups_cover_all_terms(n):
     diagram groups are a partition of the terms that writes every colour flow."""
     from paper_2312_02898_b200.gen.plan import partition_terms
     all_terms = topo.diagram_terms(n)
-    groups = partition_terms(n, max_terms=60)
+    kernels = partition_terms(n, max_terms=60, max_phase=24)
+    groups = [ph for k in kernels for ph in k]           # kernels -> phases -> terms
     assert sorted(map(repr, (t for g in groups for t in g))) == sorted(map(repr, all_terms))
     fi = topo.flow_index_table(n)
     direct = {}
@@ -109,3 +110,19 @@ def test_accumulator_blocks_reproduce_term_flows_and_groups_cover_all_terms(n):
                 for f, s in op[3]:
                     via[f] = via.get(f, 0) + abs(s) * nacc[(op[1], op[2])]
     assert via == direct and set(via) == set(range(len(fi)))
+
+
+def test_greedy_order_lowers_live_state_without_recomputation():
+    """The register-pressure-aware amplitude order (plan._greedy_order) only permutes: same currents, same FLOPs."""
+    import os
+    from paper_2312_02898_b200.gen.plan import partition_terms
+    terms = [t for ph in partition_terms(4, max_terms=40, max_phase=10 ** 6)[4] for t in ph]
+    os.environ["MG_GREEDY"] = "0"
+    try:
+        a = Plan(4, terms=terms)
+    finally:
+        os.environ["MG_GREEDY"] = "1"
+    b = Plan(4, terms=terms)
+    ca, cb = a.counts(), b.counts()
+    assert {k: ca[k] for k in ("v3", "k", "lq", "rq", "bil", "amp")} == {k: cb[k] for k in ("v3", "k", "lq", "rq", "bil", "amp")}
+    assert b.max_live() <= a.max_live()
