@@ -53,7 +53,7 @@ def config_dict(name, cfg, world, precision):
 
 
 # ---------------------------------------------------------------------------------------------- oracle legs
-ORACLE_SAMPLE = {"eemumu": 524288, "ggtt": 262144, "ggttg": 131072, "ggttgg": 49152, "ggttggg": 512}
+ORACLE_SAMPLE = {"eemumu": 524288, "ggtt": 262144, "ggttg": 131072, "ggttgg": 49152, "ggttggg": 4096}
 
 
 def oracle_time(name, cfg, nsample, repeats=1):
@@ -97,6 +97,11 @@ def run_reference(args, name, cfg):
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
     print(json.dumps(line), flush=True)
     return 0
+
+
+# DRAM bytes (read + write) moved by all kernels of one mg_sigma call at the full batch size, from ncu captures
+# (dram__bytes_read.sum + dram__bytes_write.sum summed over the launches of one call); see the named file.
+DRAM_TRAFFIC = {}
 
 
 # ---------------------------------------------------------------------------------------------- clocks
@@ -181,7 +186,6 @@ def main():
     proc.helicity_probe(mom, min(nevt, 4096))
     info = proc.info
     peak64 = mg.fma_peak(local, prec)
-    launches_per_step = proc.launches_per_sigma() + 1 if hasattr(proc, "launches_per_sigma") else 2
 
     def step(ev=None):
         if ev:
@@ -238,8 +242,12 @@ def main():
             dist.destroy_process_group()
         return 0
 
-    flops_launch = float(info.flops_per_event_goodhel) * nevt        # generator's static count (FMA = 2)
+    info = proc.info
+    launches_per_step = int(info.launches_last_sigma) + 1            # the sigma kernels + the RAMBO kernel
+    flops_launch = float(info.flops_per_event_goodhel) * nevt        # generator's static (algorithmic) count, FMA = 2
+    executed = float(info.flops_executed_per_event_goodhel) * nevt   # including diagram-group recomputation
     achieved = flops_launch * args.steps / t_sigma
+    traffic = DRAM_TRAFFIC.get((name, args.precision))
     value = nevt * world * args.steps / t_total
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
@@ -252,9 +260,15 @@ def main():
                 "api": "mg_sigma_host (pinned host momenta in, |M|^2 out)"},
         "gpu_launches": launches_per_step * args.steps,
         "roofline": {"bound": "alu", "achieved": achieved / 1e12, "peak": peak64 / 1e12, "unit": "TFLOP/s",
-                     "frac": achieved / peak64, "traffic": None,
-                     "kernel": "sigma (amplitudes + colour sum)",
+                     "frac": achieved / peak64,
+                     "traffic": None if traffic is None or args.nevt else traffic[0],
+                     "traffic_source": None if traffic is None or args.nevt else traffic[1],
+                     "kernel": "mg_sigma: all amplitude (diagram-group), gather, colour and helicity-sum kernels of one "
+                               "call, timed together with CUDA events (%d launches)" % int(info.launches_last_sigma),
                      "flops_per_event": int(info.flops_per_event_goodhel), "ngoodhel": int(info.ngoodhel),
+                     "executed_tflops": executed * args.steps / t_sigma / 1e12,
+                     "executed_frac": executed * args.steps / t_sigma / peak64,
+                     "executed_flops_per_event": int(info.flops_executed_per_event_goodhel),
                      "peak_source": "mg_fma_peak measured in this run (%s FMA loop on all SMs); MEASURED_PEAKS.json has no "
                                     "FP64 entry" % ("DFMA" if prec == mg.FP64 else "FFMA")},
         "clocks": clocks,

@@ -66,12 +66,15 @@ typedef struct {          /* caller-owned, copied by mg_process_create          
 
 typedef struct {
   int32_t npar, nfinal, ndiagrams, nhel, ngoodhel, ncolor, denominator, nepp;
-  int64_t flops_per_event_allhel;  /* generator's static FLOP count (FMA = 2), all helicities       */
-  int64_t flops_per_event_goodhel; /* same for the current good-helicity list                       */
+  int64_t flops_per_event_allhel;  /* generator's static FLOP count (FMA = 2), all helicities: the method's */
+                                   /* own (algorithmic) count, every current computed once per helicity    */
+  int64_t flops_per_event_goodhel; /* same for the current good-helicity list                              */
   double masses[8];                /* per particle, process order                                   */
   int32_t nkernels_per_tile;       /* kernel launches mg_sigma makes per event tile (1 = fused kernel)      */
-  int32_t reserved;
+  int32_t launches_last_sigma;     /* kernels launched by the last mg_sigma call on this handle             */
   int64_t workspace_bytes;         /* library-owned JAMP workspace currently allocated (split kernels only) */
+  int64_t flops_executed_per_event_goodhel; /* FLOPs the kernels execute, including the currents that      */
+                                   /* diagram-group kernels recompute (>= flops_per_event_goodhel)          */
 } mg_info_t;
 
 /* Fills *params with the defaults of BASELINE.json's configs (fp64, helicity filter, device 0). */
@@ -101,7 +104,7 @@ int mg_philox_raw(mg_process_t* p, uint64_t seed, int64_t first_event, int64_t n
  * (MG_FP32).  Asynchronous on `stream`, except that in MG_HEL_FILTER mode the first call runs the
  * helicity probe (K8) on the first min(nevt, 4096) events and synchronises the stream once, and that the
  * processes with >= 24 colour flows keep partial JAMPs in a library-owned workspace (at most MG5B200_WS_GB
- * GiB, default 16; larger batches are processed in event tiles and helicity chunks) which is (re)allocated, synchronously, by
+ * GiB, default min(64, 40 % of the free device memory); larger batches are processed in event tiles and helicity chunks) which is (re)allocated, synchronously, by
  * the first call that needs a bigger one. */
 int mg_sigma(mg_process_t* p, const void* momenta_dev, int64_t nevt, void* me_out_dev, void* stream);
 

@@ -34,8 +34,8 @@ class MgInfo(C.Structure):
     _fields_ = [("npar", C.c_int32), ("nfinal", C.c_int32), ("ndiagrams", C.c_int32), ("nhel", C.c_int32),
                 ("ngoodhel", C.c_int32), ("ncolor", C.c_int32), ("denominator", C.c_int32), ("nepp", C.c_int32),
                 ("flops_per_event_allhel", C.c_int64), ("flops_per_event_goodhel", C.c_int64),
-                ("masses", C.c_double * 8), ("nkernels_per_tile", C.c_int32), ("reserved", C.c_int32),
-                ("workspace_bytes", C.c_int64)]
+                ("masses", C.c_double * 8), ("nkernels_per_tile", C.c_int32), ("launches_last_sigma", C.c_int32),
+                ("workspace_bytes", C.c_int64), ("flops_executed_per_event_goodhel", C.c_int64)]
 
 
 class MgError(RuntimeError):

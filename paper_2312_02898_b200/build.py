@@ -18,7 +18,7 @@ OBJ = os.path.join(CSRC, "build")
 LIB = os.path.join(HERE, "libmg5b200.so")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
-FLAGS = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", "-I", CSRC]
+FLAGS = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", "-I", CSRC] + os.environ.get("MG_NVCC_EXTRA", "").split()
 
 
 def generate():

@@ -32,18 +32,25 @@ struct mg_process {
   int* hel_all_dev;        // 0..nhel-1
   std::vector<int> good;
   bool probed;
+  long long launches;      // kernels launched by the last mg_sigma / mg_sigma_per_helicity call
   void* ws;                // workspace of the split kernel shape (JAMPs + per-helicity values), library-owned
   size_t ws_bytes;
 };
 
 // Workspace for the split kernel shape: jamp[nhel_run][ncol][2][tile] + meh[nhel_run][tile]; the generated launcher
-// tiles the batch so that it fits.  Capped at MG5B200_WS_GB GiB (default 16).  Grows on demand (synchronous
+// tiles the batch so that it fits.  Capped at MG5B200_WS_GB GiB (default: min(64, 40 % of free memory)).  Grows on demand (synchronous
 // cudaFree/cudaMalloc on the first call that needs more), never shrinks.
 static int ensure_ws(mg_process* p, int64_t nevt, int nhel_run) {
   const int ip = p->par.precision == MG_FP64 ? 0 : 1;
   const size_t per_eh = (size_t)p->desc->ws_bytes_per_event_hel[ip], per_e = (size_t)p->desc->ws_bytes_per_event[ip];
   if (per_eh == 0) return MG_OK;
-  double cap_gb = 16.0;
+  // default cap: 64 GiB or 40 % of the free device memory, whichever is smaller (B200: 180 GB)
+  double cap_gb = 64.0;
+  size_t free_b = 0, total_b = 0;
+  if (cudaMemGetInfo(&free_b, &total_b) == cudaSuccess) {
+    const double f = 0.4 * (double)(free_b + p->ws_bytes) / 1073741824.0;
+    if (f < cap_gb) cap_gb = f;
+  }
   if (const char* e = getenv("MG5B200_WS_GB")) { const double v = atof(e); if (v > 0) cap_gb = v; }
   const size_t cap = (size_t)(cap_gb * 1073741824.0);
   size_t E = (size_t)((nevt + 31) / 32 * 32);
@@ -97,7 +104,7 @@ int mg_process_create(const char* proc, const mg_params_t* params, mg_process_t*
   }
   MG_CUDA(cudaSetDevice(params->device));
   mg_process* p = new mg_process();
-  p->desc = d; p->par = *params; p->probed = false; p->ws = nullptr; p->ws_bytes = 0;
+  p->desc = d; p->par = *params; p->probed = false; p->ws = nullptr; p->ws_bytes = 0; p->launches = 0;
   p->nfinal = d->npar - 2;
   for (int i = 0; i < 8; ++i) p->masses[i] = (i < d->npar && d->massive[i]) ? params->mt : 0.0;
   // derived couplings (DESIGN.md §3 C2, reading A1)
@@ -185,7 +192,7 @@ int mg_sigma_per_helicity(mg_process_t* p, const void* momenta_dev, int64_t nevt
   void* tmp = nullptr;
   { const int rc = ensure_ws(p, nevt, p->desc->nhel); if (rc != MG_OK) return rc; }
   MG_CUDA(cudaMalloc(&tmp, esize(p) * (size_t)nevt));
-  p->desc->launch(p->par.precision, (const double*)momenta_dev, tmp, nevt, p->hel_all_dev, p->desc->nhel,
+  p->launches = p->desc->launch(p->par.precision, (const double*)momenta_dev, tmp, nevt, p->hel_all_dev, p->desc->nhel,
                   perhel_out_dev, p->pvec, p->ws, p->ws_bytes, (cudaStream_t)stream);
   cudaError_t e = cudaGetLastError();
   if (e == cudaSuccess) e = cudaStreamSynchronize((cudaStream_t)stream);
@@ -237,7 +244,7 @@ int mg_sigma(mg_process_t* p, const void* momenta_dev, int64_t nevt, void* me_ou
     if (rc != MG_OK) return rc;
   }
   { const int rc = ensure_ws(p, nevt, (int)p->good.size()); if (rc != MG_OK) return rc; }
-  p->desc->launch(p->par.precision, (const double*)momenta_dev, me_out_dev, nevt, p->hel_dev, (int)p->good.size(),
+  p->launches = p->desc->launch(p->par.precision, (const double*)momenta_dev, me_out_dev, nevt, p->hel_dev, (int)p->good.size(),
                   nullptr, p->pvec, p->ws, p->ws_bytes, (cudaStream_t)stream);
   MG_CUDA(cudaGetLastError());
   return MG_OK;
@@ -279,11 +286,12 @@ int mg_process_info(const mg_process_t* p, mg_info_t* o) {
   const mg_procdesc_t* d = p->desc;
   o->npar = d->npar; o->nfinal = d->npar - 2; o->ndiagrams = d->ndiagrams; o->nhel = d->nhel;
   o->ngoodhel = (int)p->good.size(); o->ncolor = d->ncol; o->denominator = d->denominator; o->nepp = MG_NEPP;
-  o->flops_per_event_allhel = d->flops_per_helicity * d->nhel;
-  o->flops_per_event_goodhel = d->flops_per_helicity * (long long)p->good.size();
+  o->flops_per_event_allhel = d->flops_algorithmic * d->nhel;
+  o->flops_per_event_goodhel = d->flops_algorithmic * (long long)p->good.size();
+  o->flops_executed_per_event_goodhel = d->flops_per_helicity * (long long)p->good.size();
   for (int i = 0; i < 8; ++i) o->masses[i] = p->masses[i];
   o->nkernels_per_tile = d->nkernels;
-  o->reserved = 0;
+  o->launches_last_sigma = (int32_t)p->launches;
   o->workspace_bytes = (int64_t)p->ws_bytes;
   return MG_OK;
 }

@@ -30,7 +30,7 @@ MG_DEV void load_momentum(const double* __restrict__ mom, long long ievt, int ip
 // Ordered loads/stores of the per-event invariants buffer inv[item][event] (split kernel shape).  asm volatile:
 // the compiler neither hoists these out of the helicity loop nor merges repeated loads, so helicity-independent
 // operands are fetched (L1/L2) where they are used instead of living in registers or spill slots.
-#ifdef __CUDA_ARCH__
+#if defined(__CUDA_ARCH__) && !defined(MG_LDV_PLAIN)
 MG_DEV double ldv(const double* p) { double v; asm volatile("ld.global.ca.f64 %0, [%1];" : "=d"(v) : "l"(p)); return v; }
 MG_DEV float ldv(const float* p) { float v; asm volatile("ld.global.ca.f32 %0, [%1];" : "=f"(v) : "l"(p)); return v; }
 #else
@@ -52,7 +52,7 @@ template <int NPAR> MG_DEV int hel_of(int h, int ipar) {
 }
 
 #ifdef __CUDACC__
-typedef void (*mg_launch_fn)(int prec, const double* mom, void* me_out, long long nevt, const int* hel_list,
+typedef int (*mg_launch_fn)(int prec, const double* mom, void* me_out, long long nevt, const int* hel_list,
                              int nhel_run, void* perhel_out, const double* par, void* ws, size_t ws_bytes,
                              cudaStream_t st);
 struct mg_procdesc_t {
@@ -65,5 +65,8 @@ struct mg_procdesc_t {
   int nkernels;              // kernel launches per event tile (diagram groups + colour + helicity sum)
   int has_fp32;              // fp32 kernels were generated
   int ws_bytes_per_event[2]; // workspace bytes per event (helicity-independent invariants) for fp64 / fp32
+  long long flops_algorithmic;    // static count per helicity pass with every current computed once (no diagram-group
+                                  // recomputation): the method's own FLOPs; flops_per_helicity is what the kernels execute
 };
+// mg_launch_fn returns the number of kernels it launched.
 #endif  // __CUDACC__

@@ -89,7 +89,9 @@ template <class T> MG_DEV void ext_gluon(const P4<T>& k, int lambda, bool conj, 
 
 // Two-component helicity eigenspinors chi_+(p), chi_-(p) (unit norm).
 template <class T> MG_DEV void chi_pm(const P4<T>& p, T pp, C1<T> cp[2], C1<T> cm[2]) {
-  T s = pp + p.c[3];
+  // |p| + pz without cancellation for backward momenta: (|p| + pz)(|p| - pz) = kT^2
+  const T kt2 = p.c[1] * p.c[1] + p.c[2] * p.c[2];
+  T s = (p.c[3] >= T(0)) ? pp + p.c[3] : kt2 / (pp - p.c[3]);
   if (pp == T(0)) {                       // at rest: quantise along +z
     cp[0] = {T(1), T(0)}; cp[1] = {T(0), T(0)};
     cm[0] = {T(0), T(0)}; cm[1] = {T(1), T(0)};

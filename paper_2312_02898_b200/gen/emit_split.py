@@ -203,7 +203,7 @@ def _main_unit(E, n, ns, proc, npar, nhel, ncol, ndiag, cfi, cfden, union, inv, 
     w("}\n")
     w("""
 template <class T>
-static void run(const double* mom, T* me_out, long long nevt, const int* hel_list, int nhel_run, T* perhel_out,
+static int run(const double* mom, T* me_out, long long nevt, const int* hel_list, int nhel_run, T* perhel_out,
                 const double* par, void* ws, size_t ws_bytes, cudaStream_t st, int prec) {
   double norm = 1.0;
   for (int i = 0; i < NGLU; ++i) norm *= par[0];          // par[0] = g_s^2, par[1] = mt
@@ -215,9 +215,11 @@ static void run(const double* mom, T* me_out, long long nevt, const int* hel_lis
   long long E = (nevt + 31) / 32 * 32;
   if (E > 131072) E = 131072;
   while (E > 1024 && (size_t)E * (per_e + 4 * per_eh) > ws_bytes) E = (E / 2 + 1023) / 1024 * 1024;
-  if ((size_t)E * (per_e + per_eh) > ws_bytes) return;              // mg_api.cu sizes the workspace; cannot happen
+  if ((size_t)E * (per_e + per_eh) > ws_bytes) return 0;            // mg_api.cu sizes the workspace; cannot happen
+  int nlaunch = 0;
   long long H = (long long)((ws_bytes / (size_t)E - per_e) / per_eh);
   if (H > nhel_run) H = nhel_run;
+  if (H > 8) H = H / 4 * 4;
   const double* cft = nullptr; const short* pptr = nullptr; const short* pidx = nullptr;
   cudaGetSymbolAddress((void**)&cft, cf_table);
   cudaGetSymbolAddress((void**)&pptr, part_ptr);
@@ -230,33 +232,39 @@ static void run(const double* mom, T* me_out, long long nevt, const int* hel_lis
     const long long ne = nevt - e0 < E ? nevt - e0 : E;
     const double* m0 = mom + e0 * NPAR * 4;       // tile starts on a page boundary
     invariants_kernel<T><<<(unsigned)((ne + 127) / 128), 128, 0, st>>>(m0, ne, inv, E, par[1]);
+    ++nlaunch;
     for (int h0 = 0; h0 < nhel_run; h0 += (int)H) {
       const int hc = nhel_run - h0 < H ? nhel_run - h0 : (int)H;
-      // helicities per thread: keep >= ~4 waves of threads in flight
-      long long slices = (148LL * 256 * 4 + ne - 1) / ne;
+      // helicities per thread: consecutive helicities of an event reuse its invariants from L1, so give each thread
+      // as many as leaves >= ~3 waves of threads in flight, in equal shares
+      long long slices = (148LL * 256 * 3 + ne - 1) / ne;
       if (slices > hc) slices = hc;
       if (slices < 1) slices = 1;
-      const int per_thread = (int)((hc + slices - 1) / slices);
+      while (hc %% slices) ++slices;          // equal shares (hc is small)
+      const int per_thread = (int)(hc / slices);
 %(calls)s
       mgc::gather_colour_sum<T, NCOL>(cft, pptr, pidx, NPART, part, jsum, meh, E, ne, hc, T(norm), me_out + e0,
                                       perhel_out ? perhel_out + (long long)h0 * nevt + e0 : (T*)nullptr, nevt, h0 == 0, st);
+      nlaunch += %(ngroups)d + 3;
     }
   }
+  return nlaunch;
 }
-static void launch(int prec, const double* mom, void* me_out, long long nevt, const int* hel_list, int nhel_run,
-                   void* perhel_out, const double* par, void* ws, size_t ws_bytes, cudaStream_t st) {
-  if (prec == 0) run<double>(mom, (double*)me_out, nevt, hel_list, nhel_run, (double*)perhel_out, par, ws, ws_bytes, st, prec);
+static int launch(int prec, const double* mom, void* me_out, long long nevt, const int* hel_list, int nhel_run,
+                  void* perhel_out, const double* par, void* ws, size_t ws_bytes, cudaStream_t st) {
+  if (prec == 0) return run<double>(mom, (double*)me_out, nevt, hel_list, nhel_run, (double*)perhel_out, par, ws, ws_bytes, st, prec);
 %(run32)s
+  return 0;
 }
 }  // namespace
 extern const mg_procdesc_t mg_desc_%(tag)s = {"%(proc)s", %(npar)d, %(nfinal)d, %(ndiag)d, %(nhel)d, %(ncol)d, %(denom)d,
-  %(flops)dLL, {0, 0, 1, 1%(gm)s}, %(ns)s::launch, {%(ws64)d, %(ws32)d}, %(nk)d, %(hasfp32)d, {%(wse64)d, %(wse32)d}};
-""" % dict(cfden=cfden, denom=denom, tag=ns[3:], proc=proc, npar=npar, nfinal=n, ndiag=ndiag, nhel=nhel, ncol=ncol,
+  %(flops)dLL, {0, 0, 1, 1%(gm)s}, %(ns)s::launch, {%(ws64)d, %(ws32)d}, %(nk)d, %(hasfp32)d, {%(wse64)d, %(wse32)d}, %(algo)dLL};
+""" % dict(ngroups=ngroups, algo=Plan(n, acc_max=6).flops_per_helicity(), cfden=cfden, denom=denom, tag=ns[3:], proc=proc, npar=npar, nfinal=n, ndiag=ndiag, nhel=nhel, ncol=ncol,
            flops=group_flops + colour_flops, gm=", 0" * (n - 2), ns=ns,
            ws64=(2 * npart + 2 * ncol + 1) * 8, ws32=(2 * npart + 2 * ncol + 1) * 4,
            nk=ngroups + 4, hasfp32=1 if fp32 else 0, wse64=ninv * 8, wse32=ninv * 4,
            calls="\n".join("      launch_group%d(prec, ne, hel_list + h0, hc, per_thread, NPART, part, inv, E, par[1], st);" % gi
                            for gi in range(ngroups)),
-           run32=("  else run<float>(mom, (float*)me_out, nevt, hel_list, nhel_run, (float*)perhel_out, par, ws, ws_bytes, st, prec);"
+           run32=("  return run<float>(mom, (float*)me_out, nevt, hel_list, nhel_run, (float*)perhel_out, par, ws, ws_bytes, st, prec);"
                   if fp32 else "")))
     return (ns + ".cu", "".join(out))

@@ -219,6 +219,14 @@ def test_sigma_fp32_tolerance(mg, oracle, name):
     ref = oracle.me_batch(cfg["proc"], ev)
     rel = np.abs(me.cpu().numpy().astype(np.float64) / ref - 1)
     assert np.median(rel) < TOL32_MED and rel.max() < TOL32_MAX, (np.median(rel), rel.max())
+    # full batch of the config: fp32 against the fp64 CUDA path (itself checked against the oracle above)
+    nfull = cfg["nevt"]
+    p64 = mg.Process(cfg["proc"])
+    momf = p64.rambo(cfg["seed"], cfg["sqrt_s"], nfull)
+    a = p64.sigma(momf, nfull).cpu().numpy()
+    b = proc.sigma(momf, nfull).cpu().numpy().astype(np.float64)
+    relf = np.abs(b / a - 1)
+    assert np.median(relf) < TOL32_MED and relf.max() < TOL32_MAX, (np.median(relf), relf.max())
 
 
 # ------------------------------------------------------------------------------------------ edges / API
