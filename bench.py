@@ -101,7 +101,8 @@ def run_reference(args, name, cfg):
 
 # DRAM bytes (read + write) moved by all kernels of one mg_sigma call at the full batch size, from ncu captures
 # (dram__bytes_read.sum + dram__bytes_write.sum summed over the launches of one call); see the named file.
-DRAM_TRAFFIC = {}
+DRAM_TRAFFIC = {("ggttgg", "fp64"): (179.7e9, "profiles/r1_launches_ggttgg.md"),
+                ("ggttggg", "fp64"): (3492e9, "profiles/r1_launches_ggttggg.md")}
 
 
 # ---------------------------------------------------------------------------------------------- clocks
@@ -175,7 +176,7 @@ def main():
     prec = mg.FP64 if args.precision == "fp64" else mg.FP32
     proc = mg.Process(cfg["proc"], precision=prec, device=local)
     nevt = cfg["nevt"]
-    first = rank * nevt
+    first, _ = mg.shard(nevt, rank, world)
     st = torch.cuda.current_stream()
     mom = proc.alloc_momenta(nevt)
     me = torch.empty(nevt, dtype=torch.float64 if prec == mg.FP64 else torch.float32, device=mom.device)
@@ -262,7 +263,9 @@ def main():
         "roofline": {"bound": "alu", "achieved": achieved / 1e12, "peak": peak64 / 1e12, "unit": "TFLOP/s",
                      "frac": achieved / peak64,
                      "traffic": None if traffic is None or args.nevt else traffic[0],
+                     "traffic_unit": "bytes per mg_sigma call (dram read + write, all its kernels)",
                      "traffic_source": None if traffic is None or args.nevt else traffic[1],
+                     "algorithmic_bytes": nevt * (32 * info.npar + me.element_size()),
                      "kernel": "mg_sigma: all amplitude (diagram-group), gather, colour and helicity-sum kernels of one "
                                "call, timed together with CUDA events (%d launches)" % int(info.launches_last_sigma),
                      "flops_per_event": int(info.flops_per_event_goodhel), "ngoodhel": int(info.ngoodhel),

@@ -202,6 +202,15 @@ class Process:
         return [int(buf[i]) for i in range(n.value)]
 
 
+def shard(nevt_per_gpu, rank, world_size=1):
+    """Weak-scaling shard of the global event stream: rank r owns the global events
+    [r * nevt_per_gpu, (r + 1) * nevt_per_gpu).  Returns (first_event, nevt).  The Philox counter is the global
+    event index, so the union over ranks equals one big batch; no collective is needed on the data path."""
+    if not (0 <= rank < world_size) or nevt_per_gpu < 0:
+        raise ValueError("bad shard")
+    return rank * nevt_per_gpu, nevt_per_gpu
+
+
 def pages_to_events(momenta, nevt, npar):
     """AoSoA pages [page][ipar][32][4] -> plain [nevt][npar][4] (layout shuffle only; torch or numpy)."""
     pages = (nevt + NEPP - 1) // NEPP
