@@ -38,6 +38,12 @@ def generate():
             kw["block"] = int(block[str(n)])
         if str(n) in maxterms:
             kw["max_terms"] = int(maxterms[str(n)])
+        if os.environ.get("MG_STAGEKB"):
+            kw["stage_kb"] = int(os.environ["MG_STAGEKB"])
+        if os.environ.get("MG_NOINLINE"):
+            kw["noinline"] = os.environ["MG_NOINLINE"] == "1"
+        if os.environ.get("MG_FLAT"):
+            kw["flat_phase"] = int(os.environ["MG_FLAT"])
         if os.environ.get("MG_LIVEMAX"):
             kw["live_max"] = int(os.environ["MG_LIVEMAX"])
         if os.environ.get("MG_SYNC"):

@@ -36,6 +36,23 @@ MG_DEV float ldv(const float* p) { float v; asm volatile("ld.global.ca.f32 %0, [
 #else
 template <class T> MG_DEV T ldv(const T* p) { return *p; }
 #endif
+// ordered shared-memory loads (invariants staged in shared memory by a diagram-group kernel's prologue)
+#if defined(__CUDA_ARCH__)
+MG_DEV double lds(const double* p) {
+  double v; asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"((unsigned)__cvta_generic_to_shared(p))); return v;
+}
+MG_DEV float lds(const float* p) {
+  float v; asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"((unsigned)__cvta_generic_to_shared(p))); return v;
+}
+#else
+template <class T> MG_DEV T lds(const T* p) { return *p; }
+#endif
+template <class T> MG_DEV mgw::P4<T> ldps(const T* p, int blk) {
+  mgw::P4<T> o;
+#pragma unroll
+  for (int m = 0; m < 4; ++m) o.c[m] = lds(p + m * blk);
+  return o;
+}
 template <class T> MG_DEV mgw::P4<T> ldp(const T* p, long long stride) {
   mgw::P4<T> o;
 #pragma unroll

@@ -303,6 +303,16 @@ MG_DEV void cur_rq(const W4<T>& R, const W4<T>& j, const P4<T>& q, T m, T s, W4<
   o.i[3] = ms * tl1.i + qm * tu1.i + sq1 * tu0.i + sq2 * tu0.r;
 }
 
+// Out-of-line variants (experiment MG_NOINLINE_ROUTINES): by-value arguments and result, so that the device ABI can
+// keep them in registers; the kernel body becomes a sequence of calls and its instruction footprint shrinks.
+#if defined(__CUDACC__) && defined(MG_NOINLINE_ROUTINES)
+#define MG_NOINL __device__ __noinline__
+template <class T> MG_NOINL W4<T> nl_v3(P4<T> PA, W4<T> jA, P4<T> PB, W4<T> jB, T s) { W4<T> o; cur_v3(PA, jA, PB, jB, s, o); return o; }
+template <class T> MG_NOINL W4<T> nl_k(W4<T> A, W4<T> M, W4<T> C, T s) { W4<T> o; cur_k(A, M, C, s, o); return o; }
+template <class T> MG_NOINL W4<T> nl_lq(W4<T> L, W4<T> j, P4<T> q, T m, T s) { W4<T> o; cur_lq(L, j, q, m, s, o); return o; }
+template <class T> MG_NOINL W4<T> nl_rq(W4<T> R, W4<T> j, P4<T> q, T m, T s) { W4<T> o; cur_rq(R, j, q, m, s, o); return o; }
+#endif
+
 // ---------------------------------------------------------------------------------------------
 // K5: amplitudes.  The closing quark-gluon vertex  L jslash R = B_mu j^mu  with the bilinear
 // B_mu = L gamma_mu R (index lowered) shared by every diagram that closes on the same (L, R).
@@ -340,6 +350,10 @@ template <class T> MG_DEV C1<T> contract(const W4<T>& B, const W4<T>& j) {
   }
   return d;
 }
+
+#if defined(__CUDACC__) && defined(MG_NOINLINE_ROUTINES)
+template <class T> MG_NOINL W4<T> nl_bil(W4<T> L, W4<T> R) { W4<T> o; bilinear(L, R, o); return o; }
+#endif
 
 // Chiral halves of the bilinear (config 1, Z couplings):  BL_mu = L gamma_mu P_L R,  BR_mu = L gamma_mu P_R R
 // (P_L = upper two components in the Weyl basis); index lowered as in bilinear().

@@ -44,7 +44,8 @@ def choose_kernels(n, max_terms, live_max, acc_max, flat_phase=0):
 TUNED = {4: dict(max_terms=40, live_max=1000, flat_phase=0), 5: dict(max_terms=170, live_max=12, flat_phase=32)}
 
 
-def emit_split(n, block=128, fp32=True, acc_max=6, max_terms=None, sync_every=2, minblocks=2, live_max=None, flat_phase=None):
+def emit_split(n, block=128, fp32=True, acc_max=6, max_terms=None, sync_every=2, minblocks=2, live_max=None, flat_phase=None, noinline=False,
+               stage_kb=110):
     from . import emit as E
     tuned = TUNED.get(n, TUNED[5])
     max_terms = max_terms or tuned["max_terms"]
@@ -82,12 +83,29 @@ def emit_split(n, block=128, fp32=True, acc_max=6, max_terms=None, sync_every=2,
         while 2 * len(touched) * gblock * 8 > 225 * 1024:
             gblock -= 32
         smem64 = 2 * len(touched) * gblock * 8
-        gmin = min(minblocks, 2 if 2 * (smem64 + 1024) <= 227 * 1024 else 1)
+        # invariants staged in shared memory: as many of the most used items as fit next to the partial JAMPs while
+        # two CTAs still share an SM (stage_kb per CTA); the rest stays in the global buffer
+        probe = E.InvAccess(inv)
+        E._externals(_AllExternals(n), lambda x: None, probe)
+        for plan in phases:
+            E._body(plan, lambda x: None, lambda *a: None, probe)
+        budget = max(0, (stage_kb * 1024 - smem64) // (8 * gblock)) if stage_kb else 0
+        staged, nstage = {}, 0
+        for name in sorted(probe.count, key=lambda k_: (-probe.count[k_], k_)):
+            size = 1 if name[0] == "s" else 4
+            if nstage + size <= budget:
+                staged[name] = nstage
+                nstage += size
+        acc = E.InvAccess(inv, staged)
+        smem64 += nstage * gblock * 8
+        gmin = max(1, min(minblocks, (227 * 1024) // (smem64 + 1024)))
         out = [E.HEADER % dict(proc=proc, n=n, ndiag=ndiag, nterms=nterms, ncol=ncol, nhel=nhel, flops=flops, ns=ns,
                                npar=npar, what="diagram group %d of %d, %d phase(s) (partial JAMP slots %d..%d)"
                                % (gi, nkern, len(phases), base, base + len(touched) - 1))]
         w = out.append
-        w("constexpr int BLK = %d, NTOUCH = %d, PBASE = %d;\n" % (gblock, len(touched), base))
+        if noinline:
+            out[0] = "#define MG_NOINLINE_ROUTINES 1\n" + out[0]
+        w("constexpr int BLK = %d, NTOUCH = %d, PBASE = %d, NSTAGE = %d;\n" % (gblock, len(touched), base, nstage))
         w("template <class T>\n__global__ void __launch_bounds__(%d, %d)\n" % (gblock, gmin))
         w("group%d_kernel(long long nevt, const int* __restrict__ hel_list, int hcount, int per_thread, int npart,\n"
           "              T* __restrict__ part, const T* __restrict__ invbuf, long long stride, double mt_d) {\n" % gi)
@@ -96,10 +114,14 @@ def emit_split(n, block=128, fp32=True, acc_max=6, max_terms=None, sync_every=2,
         w("  const long long ievt0 = (long long)blockIdx.x * blockDim.x + threadIdx.x;\n")
         w("  const bool live = ievt0 < nevt;\n  const long long ievt = live ? ievt0 : nevt - 1;\n")
         w("  const T* __restrict__ inv = invbuf + ievt;\n  const T mt = T(mt_d);\n")
+        w("  T* __restrict__ sinv = sj + 2 * NTOUCH * BLK;    // staged invariants, sinv[slot][thread]\n")
+        for name, sl in sorted(staged.items(), key=lambda kv: kv[1]):
+            for m in range(1 if name[0] == "s" else 4):
+                w("  sinv[%d * BLK] = inv[%d * stride];\n" % (sl + m, inv[name] + m))
         w("  const int ih0 = blockIdx.y * per_thread, ih1 = min(hcount, ih0 + per_thread);\n")
         w("#pragma unroll 1\n  for (int ih = ih0; ih < ih1; ++ih) {\n")
         w("    const int h = hel_list[ih];\n")
-        E._externals(_AllExternals(n), w, inv)
+        E._externals(_AllExternals(n), w, acc)
         local_written = set()
 
         def sink(f, s, re, im, slot=slot, local_written=local_written, w=w):
@@ -114,7 +136,7 @@ def emit_split(n, block=128, fp32=True, acc_max=6, max_terms=None, sync_every=2,
 
         for pi, plan in enumerate(phases):
             w("    {   // phase %d: %d terms, <= %d live currents\n" % (pi, len(plan.terms), plan.max_live()))
-            E._body(plan, w, sink, inv, sync_every=sync_every)
+            E._body(plan, w, sink, acc, sync_every=sync_every, noinline=noinline)
             w("    }\n")
         w("    if (live) {\n")
         w("      T* __restrict__ pb = part + ((long long)ih * npart + PBASE) * 2 * stride + ievt;\n")
@@ -124,17 +146,18 @@ def emit_split(n, block=128, fp32=True, acc_max=6, max_terms=None, sync_every=2,
           "                    const void* inv, long long stride, double mt, cudaStream_t st) {\n" % gi)
         w("  const dim3 grid((unsigned)((nevt + BLK - 1) / BLK), (unsigned)((hcount + per_thread - 1) / per_thread));\n")
         w("  static bool attr_set = false;\n  if (!attr_set) {\n")
-        w("    cudaFuncSetAttribute(group%d_kernel<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * NTOUCH * BLK * 8);\n" % gi)
+        w("    cudaFuncSetAttribute(group%d_kernel<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (2 * NTOUCH + NSTAGE) * BLK * 8);\n" % gi)
         if fp32:
-            w("    cudaFuncSetAttribute(group%d_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * NTOUCH * BLK * 4);\n" % gi)
+            w("    cudaFuncSetAttribute(group%d_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (2 * NTOUCH + NSTAGE) * BLK * 4);\n" % gi)
         w("    attr_set = true;\n  }\n")
-        w("  if (prec == 0) group%d_kernel<double><<<grid, BLK, 2 * NTOUCH * BLK * 8, st>>>(nevt, hel_list, hcount, per_thread, npart, (double*)part, (const double*)inv, stride, mt);\n" % gi)
+        w("  if (prec == 0) group%d_kernel<double><<<grid, BLK, (2 * NTOUCH + NSTAGE) * BLK * 8, st>>>(nevt, hel_list, hcount, per_thread, npart, (double*)part, (const double*)inv, stride, mt);\n" % gi)
         if fp32:
-            w("  else group%d_kernel<float><<<grid, BLK, 2 * NTOUCH * BLK * 4, st>>>(nevt, hel_list, hcount, per_thread, npart, (float*)part, (const float*)inv, stride, mt);\n" % gi)
+            w("  else group%d_kernel<float><<<grid, BLK, (2 * NTOUCH + NSTAGE) * BLK * 4, st>>>(nevt, hel_list, hcount, per_thread, npart, (float*)part, (const float*)inv, stride, mt);\n" % gi)
         w("}\n}  // namespace\n")
         files.append(("%s_g%02d.cu" % (ns, gi), "".join(out)))
         ginfo.append(dict(terms=nterms, phases=[len(p.terms) for p in phases], max_live=live, flops=flops,
-                          flows=len(touched), block=gblock, minblocks=gmin, smem64=smem64))
+                          flows=len(touched), block=gblock, minblocks=gmin, smem64=smem64, staged=nstage,
+                          inv_items=sum(1 if k_[0] == "s" else 4 for k_ in probe.count)))
         base += len(touched)
     npart = base
     assert all(part_of_flow[f] for f in range(ncol)), "every colour flow must be written by some group"
