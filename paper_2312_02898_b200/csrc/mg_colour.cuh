@@ -175,7 +175,7 @@ __global__ void __launch_bounds__(PAIRS * GROUPS) gather_colour_kernel(const dou
 template <class T, int NCOL>
 void gather_colour_sum(const double* cft, const short* ptr, const short* idx, int npart, const T* part, T* jsum, T* meh,
                        long long stride, long long nevt, int nhel_run, T norm, T* me_out, T* perhel_out,
-                       long long perhel_stride, bool first, cudaStream_t st) {
+                       long long perhel_stride, bool first, bool gather, cudaStream_t st) {
   // NCOL <= 32: one thread per pair does everything (128 pairs per CTA); larger bases: 32 pairs x 5 groups
   constexpr int PAIRS = NCOL <= 32 ? 128 : 32, GROUPS = NCOL <= 32 ? 1 : 5;
   const size_t smem = (size_t)(2 * NCOL + GROUPS) * PAIRS * sizeof(T);
@@ -187,9 +187,13 @@ void gather_colour_sum(const double* cft, const short* ptr, const short* idx, in
   auto kern = gather_colour_kernel<T, NCOL, PAIRS, GROUPS, false>;
   if (!attr_set) { cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); attr_set = true; }
   kern<<<grid, PAIRS * GROUPS, smem, st>>>(cft, ptr, idx, npart, part, meh, stride, nevt);
+  (void)gather;
 #else
-  const dim3 g1((unsigned)((nevt + 255) / 256), (unsigned)nhel_run);
-  gather_kernel<T, NCOL><<<g1, 256, 0, st>>>(ptr, idx, npart, part, jsum, stride, nevt);
+  // gather == false: the diagram-group kernels accumulated the JAMPs in place (jsum == part, npart == NCOL)
+  if (gather) {
+    const dim3 g1((unsigned)((nevt + 255) / 256), (unsigned)nhel_run);
+    gather_kernel<T, NCOL><<<g1, 256, 0, st>>>(ptr, idx, npart, part, jsum, stride, nevt);
+  }
   if (NCOL > 32) {
     // large colour basis: JAMPs staged once in shared memory (the plain kernel re-reads them 7.7x from DRAM at
     // NCOL = 120); measured +3 % on gg->tt~ggg, -1 % on gg->tt~gg (NCOL = 24, where the plain kernel stays)

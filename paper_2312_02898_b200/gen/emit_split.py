@@ -40,12 +40,12 @@ def choose_kernels(n, max_terms, live_max, acc_max, flat_phase=0):
 
 # measured on B200: short kernels win — their straight-line bodies stay in the instruction caches and
 # their live state fits the register file — even though every extra kernel recomputes a few shared currents and
-# adds partial-JAMP slots.  n = 4: 8 kernels of <= 40 terms; n = 5: 63 kernels of <= 32 terms.
-TUNED = {4: dict(max_terms=40, live_max=1000, flat_phase=0), 5: dict(max_terms=170, live_max=12, flat_phase=32)}
+# adds partial-JAMP slots.  n = 4: 8 kernels of <= 40 terms; n = 5: 80 kernels of <= 24 terms.
+TUNED = {4: dict(max_terms=40, live_max=1000, flat_phase=0), 5: dict(max_terms=170, live_max=12, flat_phase=24)}
 
 
 def emit_split(n, block=128, fp32=True, acc_max=6, max_terms=None, sync_every=2, minblocks=2, live_max=None, flat_phase=None, noinline=False,
-               stage_kb=110):
+               stage_kb=110, reduce_mode="red"):
     from . import emit as E
     tuned = TUNED.get(n, TUNED[5])
     max_terms = max_terms or tuned["max_terms"]
@@ -67,6 +67,7 @@ def emit_split(n, block=128, fp32=True, acc_max=6, max_terms=None, sync_every=2,
     files, ginfo = [], []
     total_flops = 0
     part_of_flow = {f: [] for f in range(ncol)}     # flow -> global partial slots
+    written_flows = set()                            # reduce_mode "red": flows some earlier kernel has stored
     base = 0
     nkern = len(kernels)
     ext_flops = Plan(n, terms=[]).flops_per_helicity(colour=False)      # external wavefunctions, once per kernel
@@ -79,6 +80,8 @@ def emit_split(n, block=128, fp32=True, acc_max=6, max_terms=None, sync_every=2,
         slot = {f: i for i, f in enumerate(touched)}
         for f in touched:
             part_of_flow[f].append(base + slot[f])
+        first_writer = [f for f in touched if f not in written_flows]
+        written_flows.update(touched)
         gblock = block
         while 2 * len(touched) * gblock * 8 > 225 * 1024:
             gblock -= 32
@@ -139,8 +142,20 @@ def emit_split(n, block=128, fp32=True, acc_max=6, max_terms=None, sync_every=2,
             E._body(plan, w, sink, acc, sync_every=sync_every, noinline=noinline)
             w("    }\n")
         w("    if (live) {\n")
-        w("      T* __restrict__ pb = part + ((long long)ih * npart + PBASE) * 2 * stride + ievt;\n")
-        w("#pragma unroll\n      for (int q = 0; q < 2 * NTOUCH; ++q) pb[q * stride] = sj[q * BLK];\n")
+        if reduce_mode == "red":
+            # JAMP[f] accumulated in place across the kernels of the stream: the first kernel (in launch order) that
+            # touches a flow stores, the later ones add with fire-and-forget L2 reductions (red.global.add): no
+            # partial slots, no gather pass, and still a fixed summation order (one add per kernel, stream order)
+            w("      T* __restrict__ pb = part + (long long)ih * npart * 2 * stride + ievt;\n")
+            for f in touched:
+                for c_ in (0, 1):
+                    if f in first_writer:
+                        w("      pb[%d * stride] = sj[%d * BLK];\n" % (2 * f + c_, 2 * slot[f] + c_))
+                    else:
+                        w("      atomicAdd(pb + %d * stride, sj[%d * BLK]);\n" % (2 * f + c_, 2 * slot[f] + c_))
+        else:
+            w("      T* __restrict__ pb = part + ((long long)ih * npart + PBASE) * 2 * stride + ievt;\n")
+            w("#pragma unroll\n      for (int q = 0; q < 2 * NTOUCH; ++q) pb[q * stride] = sj[q * BLK];\n")
         w("    }\n  }\n}\n")
         w("void launch_group%d(int prec, long long nevt, const int* hel_list, int hcount, int per_thread, int npart, void* part,\n"
           "                    const void* inv, long long stride, double mt, cudaStream_t st) {\n" % gi)
@@ -159,10 +174,10 @@ def emit_split(n, block=128, fp32=True, acc_max=6, max_terms=None, sync_every=2,
                           flows=len(touched), block=gblock, minblocks=gmin, smem64=smem64, staged=nstage,
                           inv_items=sum(1 if k_[0] == "s" else 4 for k_ in probe.count)))
         base += len(touched)
-    npart = base
+    npart = base if reduce_mode != "red" else ncol
     assert all(part_of_flow[f] for f in range(ncol)), "every colour flow must be written by some group"
     files.append(_main_unit(E, n, ns, proc, npar, nhel, ncol, ndiag, cfi, cfden, union, inv, ninv, npart, part_of_flow,
-                            nkern, total_flops, fp32))
+                            nkern, total_flops, fp32, reduce_mode))
     colour_flops = 2 * (ncol * (ncol - 1) // 2) * 2 + ncol * 8
     info = dict(proc=proc, ns=ns, npar=npar, ncol=ncol, nhel=nhel, ndiagrams=ndiag, nterms=sum(len(p.terms) for p in plans),
                 flops_per_helicity=total_flops + colour_flops, shape="split", ngroups=nkern, npart=npart, ninv=ninv,
@@ -179,7 +194,7 @@ class _AllExternals:
 
 
 def _main_unit(E, n, ns, proc, npar, nhel, ncol, ndiag, cfi, cfden, union, inv, ninv, npart, part_of_flow, ngroups,
-               group_flops, fp32):
+               group_flops, fp32, reduce_mode="slots"):
     colour_flops = 2 * (ncol * (ncol - 1) // 2) * 2 + ncol * 8
     denom = 4 * 64 * factorial(n - 2)
     rows = E._colour_rows(cfi, ncol)
@@ -232,7 +247,7 @@ static int run(const double* mom, T* me_out, long long nevt, const int* hel_list
   for (int i = 0; i < NGLU; ++i) norm *= par[0];          // par[0] = g_s^2, par[1] = mt
   norm /= (double)%(cfden)d * (double)%(denom)d;
   const size_t es = sizeof(T);
-  const size_t per_eh = (size_t)(2 * NPART + 2 * NCOL + 1) * es;     // bytes per (event, helicity)
+  const size_t per_eh = (size_t)(%(slots)s + 2 * NCOL + 1) * es;     // bytes per (event, helicity)
   const size_t per_e = (size_t)NINV * es;                            // bytes per event
   // event tile E (multiple of 1024, or the whole padded batch) and helicity chunk H
   long long E = (nevt + 31) / 32 * 32;
@@ -248,7 +263,7 @@ static int run(const double* mom, T* me_out, long long nevt, const int* hel_list
   cudaGetSymbolAddress((void**)&pptr, part_ptr);
   cudaGetSymbolAddress((void**)&pidx, part_idx);
   T* part = (T*)ws;
-  T* jsum = part + (size_t)H * 2 * NPART * E;
+  T* jsum = part + (size_t)H * %(slots)s * E;
   T* meh = jsum + (size_t)H * 2 * NCOL * E;
   T* inv = meh + (size_t)H * E;
   for (long long e0 = 0; e0 < nevt; e0 += E) {
@@ -266,9 +281,9 @@ static int run(const double* mom, T* me_out, long long nevt, const int* hel_list
       while (hc %% slices) ++slices;          // equal shares (hc is small)
       const int per_thread = (int)(hc / slices);
 %(calls)s
-      mgc::gather_colour_sum<T, NCOL>(cft, pptr, pidx, NPART, part, jsum, meh, E, ne, hc, T(norm), me_out + e0,
-                                      perhel_out ? perhel_out + (long long)h0 * nevt + e0 : (T*)nullptr, nevt, h0 == 0, st);
-      nlaunch += %(ngroups)d + 3;
+      mgc::gather_colour_sum<T, NCOL>(cft, pptr, pidx, NPART, part, %(jsrc)s, meh, E, ne, hc, T(norm), me_out + e0,
+                                      perhel_out ? perhel_out + (long long)h0 * nevt + e0 : (T*)nullptr, nevt, h0 == 0, %(gather)s, st);
+      nlaunch += %(ngroups)d + %(extra)d;
     }
   }
   return nlaunch;
@@ -284,8 +299,11 @@ extern const mg_procdesc_t mg_desc_%(tag)s = {"%(proc)s", %(npar)d, %(nfinal)d, 
   %(flops)dLL, {0, 0, 1, 1%(gm)s}, %(ns)s::launch, {%(ws64)d, %(ws32)d}, %(nk)d, %(hasfp32)d, {%(wse64)d, %(wse32)d}, %(algo)dLL};
 """ % dict(ngroups=ngroups, algo=Plan(n, acc_max=6).flops_per_helicity(), cfden=cfden, denom=denom, tag=ns[3:], proc=proc, npar=npar, nfinal=n, ndiag=ndiag, nhel=nhel, ncol=ncol,
            flops=group_flops + colour_flops, gm=", 0" * (n - 2), ns=ns,
-           ws64=(2 * npart + 2 * ncol + 1) * 8, ws32=(2 * npart + 2 * ncol + 1) * 4,
-           nk=ngroups + 4, hasfp32=1 if fp32 else 0, wse64=ninv * 8, wse32=ninv * 4,
+           ws64=((0 if reduce_mode == "red" else 2 * npart) + 2 * ncol + 1) * 8,
+           ws32=((0 if reduce_mode == "red" else 2 * npart) + 2 * ncol + 1) * 4,
+           slots="0" if reduce_mode == "red" else "2 * NPART", jsrc="part" if reduce_mode == "red" else "jsum",
+           gather="false" if reduce_mode == "red" else "true", extra=2 if reduce_mode == "red" else 3,
+           nk=ngroups + (3 if reduce_mode == "red" else 4), hasfp32=1 if fp32 else 0, wse64=ninv * 8, wse32=ninv * 4,
            calls="\n".join("      launch_group%d(prec, ne, hel_list + h0, hc, per_thread, NPART, part, inv, E, par[1], st);" % gi
                            for gi in range(ngroups)),
            run32=("  return run<float>(mom, (float*)me_out, nevt, hel_list, nhel_run, (float*)perhel_out, par, ws, ws_bytes, st, prec);"
