@@ -22,6 +22,8 @@ def choose_kernels(n, max_terms, live_max, acc_max, flat_phase=0):
     phase recomputes the low-multiplicity currents it shares with its neighbours."""
     import os
     flat = int(os.environ.get("MG_FLATPHASE", "0")) or flat_phase
+    if flat and os.environ.get("MG_FLAT_LR"):
+        flat = {"*": flat, "L": int(os.environ["MG_FLAT_LR"]), "R": int(os.environ["MG_FLAT_LR"])}
     if flat:
         # every phase its own kernel: short straight-line bodies that stay resident in the instruction caches
         return [[Plan(n, terms=ph, acc_max=acc_max)] for k in partition_terms(n, max_terms=max_terms, max_phase=flat)

@@ -462,11 +462,18 @@ def group_key(term, n):
         return ("A", tuple(sorted(la))), big_child(anc)
     if len(la) >= n:
         return ("T", mid[0]), big_child(mid)
+    # quark-line dominated terms: keyed by the gluon *set* on the top side of the closing block (the terms of a set
+    # share all their top-side chains and need antitop-side chains over the complement only), then by the closing
+    # block; terms closed on their first block are keyed by that block
+    def mask(ts):
+        out = ()
+        for t in ts:
+            out += tuple(topo.leaves_of(t))
+        return tuple(sorted(out))
+
     if c > 0:
-        nxt = tuple(sorted(topo.leaves_of(term[1])))
-        return ("L", tuple(sorted(topo.leaves_of(term[0])))), nxt
-    prv = tuple(sorted(topo.leaves_of(term[-2]))) if len(term) > 1 else ()
-    return ("R", tuple(sorted(topo.leaves_of(term[-1])))), prv
+        return ("L", mask(term[:c])), tuple(sorted(topo.leaves_of(mid)))
+    return ("R", tuple(sorted(topo.leaves_of(mid)))), mask(term[c + 1:c + 2])
 
 
 def amp_sort_key(lchain, rchain, mid, acc_max, n):
@@ -510,7 +517,9 @@ def partition_terms(n, max_terms=170, max_phase=32):
         out, cur = [], []
         for fk in sorted(fine, key=repr):
             b = fine[fk]
-            if cur and len(cur) + len(b) > max_phase:
+            cls = fk[0][0] if isinstance(fk[0], tuple) else fk[0]
+            limit = max_phase.get(cls, max_phase.get("*", 32)) if isinstance(max_phase, dict) else max_phase
+            if cur and len(cur) + len(b) > limit:
                 out.append(cur)
                 cur = []
             cur = cur + b
