@@ -72,7 +72,7 @@ def emit_split(n, block=128, fp32=True, acc_max=6, max_terms=None, sync_every=2,
     written_flows = set()                            # reduce_mode "red": flows some earlier kernel has stored
     base = 0
     nkern = len(kernels)
-    ext_flops = Plan(n, terms=[]).flops_per_helicity(colour=False)      # external wavefunctions, once per kernel
+    ext_flops = 0      # external wavefunctions come from per-event tables (invariants kernel): no FLOPs per helicity
     for gi, phases in enumerate(kernels):
         flops = sum(p.flops_per_helicity(colour=False, externals=False) for p in phases) + ext_flops
         total_flops += flops
@@ -90,18 +90,18 @@ def emit_split(n, block=128, fp32=True, acc_max=6, max_terms=None, sync_every=2,
         smem64 = 2 * len(touched) * gblock * 8
         # invariants staged in shared memory: as many of the most used items as fit next to the partial JAMPs while
         # two CTAs still share an SM (stage_kb per CTA); the rest stays in the global buffer
-        probe = E.InvAccess(inv)
+        probe = E.InvAccess(inv, union.sizes)
         E._externals(_AllExternals(n), lambda x: None, probe)
         for plan in phases:
             E._body(plan, lambda x: None, lambda *a: None, probe)
         budget = max(0, (stage_kb * 1024 - smem64) // (8 * gblock)) if stage_kb else 0
         staged, nstage = {}, 0
         for name in sorted(probe.count, key=lambda k_: (-probe.count[k_], k_)):
-            size = 1 if name[0] == "s" else 4
+            size = union.sizes[name]
             if nstage + size <= budget:
                 staged[name] = nstage
                 nstage += size
-        acc = E.InvAccess(inv, staged)
+        acc = E.InvAccess(inv, union.sizes, staged)
         smem64 += nstage * gblock * 8
         gmin = max(1, min(minblocks, (227 * 1024) // (smem64 + 1024)))
         out = [E.HEADER % dict(proc=proc, n=n, ndiag=ndiag, nterms=nterms, ncol=ncol, nhel=nhel, flops=flops, ns=ns,
@@ -121,7 +121,7 @@ def emit_split(n, block=128, fp32=True, acc_max=6, max_terms=None, sync_every=2,
         w("  const T* __restrict__ inv = invbuf + ievt;\n  const T mt = T(mt_d);\n")
         w("  T* __restrict__ sinv = sj + 2 * NTOUCH * BLK;    // staged invariants, sinv[slot][thread]\n")
         for name, sl in sorted(staged.items(), key=lambda kv: kv[1]):
-            for m in range(1 if name[0] == "s" else 4):
+            for m in range(union.sizes[name]):
                 w("  sinv[%d * BLK] = inv[%d * stride];\n" % (sl + m, inv[name] + m))
         w("  const int ih0 = blockIdx.y * per_thread, ih1 = min(hcount, ih0 + per_thread);\n")
         w("#pragma unroll 1\n  for (int ih = ih0; ih < ih1; ++ih) {\n")
@@ -174,7 +174,7 @@ def emit_split(n, block=128, fp32=True, acc_max=6, max_terms=None, sync_every=2,
         files.append(("%s_g%02d.cu" % (ns, gi), "".join(out)))
         ginfo.append(dict(terms=nterms, phases=[len(p.terms) for p in phases], max_live=live, flops=flops,
                           flows=len(touched), block=gblock, minblocks=gmin, smem64=smem64, staged=nstage,
-                          inv_items=sum(1 if k_[0] == "s" else 4 for k_ in probe.count)))
+                          inv_items=sum(union.sizes[k_] for k_ in probe.count)))
         base += len(touched)
     npart = base if reduce_mode != "red" else ncol
     assert all(part_of_flow[f] for f in range(ncol)), "every colour flow must be written by some group"
@@ -237,9 +237,19 @@ def _main_unit(E, n, ns, proc, npar, nhel, ncol, ndiag, cfi, cfden, union, inv, 
     for name, i in sorted(inv.items(), key=lambda kv: kv[1]):
         if name[0] == "s":
             w("  o[%d * stride] = %s;\n" % (i, name))
+        elif name.startswith("eg"):
+            g = int(name[2:])
+            w("  { W4<double> e; ext_gluon(kd[%d], +1, %s, e);   // lambda = +1: e.r = -R, e.i = I\n" % (g, "false" if g < 2 else "true"))
+            w("    o[%d * stride] = T(-e.r[1]); o[%d * stride] = T(-e.r[2]); o[%d * stride] = T(-e.r[3]);\n" % (i, i + 1, i + 2))
+            w("    o[%d * stride] = T(e.i[1]); o[%d * stride] = T(e.i[2]); }\n" % (i + 3, i + 4))
+        elif name in ("ub", "vv"):
+            fn, mom = ("ext_ubar", "ptd") if name == "ub" else ("ext_v", "ptbd")
+            for hi, lam in ((0, "+1"), (8, "-1")):
+                w("  { W4<double> q; %s(%s, mt_d, %s, q);\n" % (fn, mom, lam))
+                w("    " + " ".join("o[%d * stride] = T(q.r[%d]); o[%d * stride] = T(q.i[%d]);"
+                                    % (i + hi + 2 * m, m, i + hi + 2 * m + 1, m) for m in range(4)) + " }\n")
         else:
-            src = "k[%s]" % name[1:] if name[0] == "k" else name
-            w("  stp(o + %d * stride, stride, %s);\n" % (i, src))
+            w("  stp(o + %d * stride, stride, %s);\n" % (i, name))
     w("}\n")
     w("""
 template <class T>
@@ -299,7 +309,7 @@ static int launch(int prec, const double* mom, void* me_out, long long nevt, con
 }  // namespace
 extern const mg_procdesc_t mg_desc_%(tag)s = {"%(proc)s", %(npar)d, %(nfinal)d, %(ndiag)d, %(nhel)d, %(ncol)d, %(denom)d,
   %(flops)dLL, {0, 0, 1, 1%(gm)s}, %(ns)s::launch, {%(ws64)d, %(ws32)d}, %(nk)d, %(hasfp32)d, {%(wse64)d, %(wse32)d}, %(algo)dLL};
-""" % dict(ngroups=ngroups, algo=Plan(n, acc_max=6).flops_per_helicity(), cfden=cfden, denom=denom, tag=ns[3:], proc=proc, npar=npar, nfinal=n, ndiag=ndiag, nhel=nhel, ncol=ncol,
+""" % dict(ngroups=ngroups, algo=Plan(n, acc_max=6).flops_per_helicity(externals=False), cfden=cfden, denom=denom, tag=ns[3:], proc=proc, npar=npar, nfinal=n, ndiag=ndiag, nhel=nhel, ncol=ncol,
            flops=group_flops + colour_flops, gm=", 0" * (n - 2), ns=ns,
            ws64=((0 if reduce_mode == "red" else 2 * npart) + 2 * ncol + 1) * 8,
            ws32=((0 if reduce_mode == "red" else 2 * npart) + 2 * ncol + 1) * 4,
