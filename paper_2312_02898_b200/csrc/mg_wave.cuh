@@ -209,6 +209,21 @@ MG_DEV void cur_v3(const P4<T>& PA, const W4<T>& jA, const P4<T>& PB, const W4<T
   }
 }
 
+// Same current from helicity-independent vectors prepared once per event (split kernel shape):
+//   sdp = s (PA - PB),  sqa = s (2 PB + PA),  sqb = -s (2 PA + PB),  s = -1/(PA+PB)^2
+//   j = (jA.jB) sdp + (sqa.jA) jB + (sqb.jB) jA
+template <class T>
+MG_DEV void cur_v3p(const W4<T>& jA, const W4<T>& jB, const P4<T>& sdp, const P4<T>& sqa, const P4<T>& sqb, W4<T>& o) {
+  const C1<T> d = wdot(jA, jB);
+  const C1<T> a = pwdot(sqa, jA);
+  const C1<T> b = pwdot(sqb, jB);
+#pragma unroll
+  for (int m = 0; m < 4; ++m) {
+    o.r[m] = d.r * sdp.c[m] + a.r * jB.r[m] - a.i * jB.i[m] + b.r * jA.r[m] - b.i * jA.i[m];
+    o.i[m] = d.i * sdp.c[m] + a.r * jB.i[m] + a.i * jB.r[m] + b.r * jA.i[m] + b.i * jA.r[m];
+  }
+}
+
 // gggg kinematic structure with M in the middle:  j = s * [(A.M) C + (M.C) A - 2 (A.C) M],  s = -1/P^2.
 template <class T>
 MG_DEV void cur_k(const W4<T>& A, const W4<T>& M, const W4<T>& C, T s, W4<T>& o) {
@@ -252,8 +267,16 @@ template <class T> MG_DEV void col2(const M2<T>& m, const C1<T>& x0, const C1<T>
 }
 
 // Quark-line step from the top side (row spinor):  o = s * L jslash (qslash + m),  s = -1/(q^2-m^2).
+// quark-line steps with the helicity-independent propagator factors prepared once per event (split kernel shape):
+//   qp = s (q0 + q3), qm = s (q0 - q3), sq1 = s q1, sq2 = s q2, ms = s m
+template <class T> MG_DEV void cur_lqp(const W4<T>& L, const W4<T>& j, T qp, T qm, T sq1, T sq2, T ms, W4<T>& o);
+template <class T> MG_DEV void cur_rqp(const W4<T>& R, const W4<T>& j, T qp, T qm, T sq1, T sq2, T ms, W4<T>& o);
 template <class T>
 MG_DEV void cur_lq(const W4<T>& L, const W4<T>& j, const P4<T>& q, T m, T s, W4<T>& o) {
+  cur_lqp(L, j, s * (q.c[0] + q.c[3]), s * (q.c[0] - q.c[3]), s * q.c[1], s * q.c[2], m * s, o);
+}
+template <class T>
+MG_DEV void cur_lqp(const W4<T>& L, const W4<T>& j, T qp, T qm, T sq1, T sq2, T ms, W4<T>& o) {
   M2<T> mp, mm;
   slash_blocks(j, mp, mm);
   C1<T> lu0 = {L.r[0], L.i[0]}, lu1 = {L.r[1], L.i[1]}, ll0 = {L.r[2], L.i[2]}, ll1 = {L.r[3], L.i[3]};
@@ -261,10 +284,6 @@ MG_DEV void cur_lq(const W4<T>& L, const W4<T>& j, const P4<T>& q, T m, T s, W4<
   row2(ll0, ll1, mp, tu0, tu1);      // (L jslash)_U = L_L M+(j)
   row2(lu0, lu1, mm, tl0, tl1);      // (L jslash)_L = L_U M-(j)
   // times (qslash + m), q real:  res_U = t_L M+(q) + m t_U ; res_L = t_U M-(q) + m t_L
-  T qp = q.c[0] + q.c[3], qm = q.c[0] - q.c[3];
-  T ms = m * s;
-  T sq1 = s * q.c[1], sq2 = s * q.c[2];
-  qp *= s; qm *= s;
   // M+(q) = [[qp, q1 - i q2],[q1 + i q2, qm]]
   o.r[0] = ms * tu0.r + tl0.r * qp + tl1.r * sq1 - tl1.i * sq2;
   o.i[0] = ms * tu0.i + tl0.i * qp + tl1.i * sq1 + tl1.r * sq2;
@@ -280,6 +299,10 @@ MG_DEV void cur_lq(const W4<T>& L, const W4<T>& j, const P4<T>& q, T m, T s, W4<
 // Quark-line step from the antitop side (column spinor):  o = s * (qslash + m) jslash R,  s = -1/(q^2-m^2).
 template <class T>
 MG_DEV void cur_rq(const W4<T>& R, const W4<T>& j, const P4<T>& q, T m, T s, W4<T>& o) {
+  cur_rqp(R, j, s * (q.c[0] + q.c[3]), s * (q.c[0] - q.c[3]), s * q.c[1], s * q.c[2], m * s, o);
+}
+template <class T>
+MG_DEV void cur_rqp(const W4<T>& R, const W4<T>& j, T qp, T qm, T sq1, T sq2, T ms, W4<T>& o) {
   M2<T> mp, mm;
   slash_blocks(j, mp, mm);
   C1<T> ru0 = {R.r[0], R.i[0]}, ru1 = {R.r[1], R.i[1]}, rl0 = {R.r[2], R.i[2]}, rl1 = {R.r[3], R.i[3]};
@@ -287,10 +310,6 @@ MG_DEV void cur_rq(const W4<T>& R, const W4<T>& j, const P4<T>& q, T m, T s, W4<
   col2(mm, rl0, rl1, tu0, tu1);      // (jslash R)_U = M-(j) R_L
   col2(mp, ru0, ru1, tl0, tl1);      // (jslash R)_L = M+(j) R_U
   // (qslash + m) t:  res_U = M-(q) t_L + m t_U ; res_L = M+(q) t_U + m t_L
-  T qp = q.c[0] + q.c[3], qm = q.c[0] - q.c[3];
-  T ms = m * s;
-  T sq1 = s * q.c[1], sq2 = s * q.c[2];
-  qp *= s; qm *= s;
   // M-(q) = [[qm, -q1 + i q2],[-q1 - i q2, qp]]
   o.r[0] = ms * tu0.r + qm * tl0.r - sq1 * tl1.r - sq2 * tl1.i;
   o.i[0] = ms * tu0.i + qm * tl0.i - sq1 * tl1.i + sq2 * tl1.r;

@@ -242,6 +242,19 @@ def _main_unit(E, n, ns, proc, npar, nhel, ncol, ndiag, cfi, cfden, union, inv, 
             w("  { W4<double> e; ext_gluon(kd[%d], +1, %s, e);   // lambda = +1: e.r = -R, e.i = I\n" % (g, "false" if g < 2 else "true"))
             w("    o[%d * stride] = T(-e.r[1]); o[%d * stride] = T(-e.r[2]); o[%d * stride] = T(-e.r[3]);\n" % (i, i + 1, i + 2))
             w("    o[%d * stride] = T(e.i[1]); o[%d * stride] = T(e.i[2]); }\n" % (i + 3, i + 4))
+        elif name.startswith("v3_"):
+            ma, mb = (int(x) for x in name[3:].split("_"))
+            sgn = "dsg%d" % (ma | mb)
+            for m in range(4):
+                w("  o[%d * stride] = T(%s * (dm%d.c[%d] - dm%d.c[%d])); o[%d * stride] = T(%s * (2.0 * dm%d.c[%d] + dm%d.c[%d])); "
+                  "o[%d * stride] = T(-%s * (2.0 * dm%d.c[%d] + dm%d.c[%d]));\n"
+                  % (i + m, sgn, ma, m, mb, m, i + 4 + m, sgn, mb, m, ma, m, i + 8 + m, sgn, ma, m, mb, m))
+        elif name.startswith("tl") or name.startswith("tr"):
+            side, m_ = name[1], int(name[2:])
+            sv, qv = "ds%s%d" % (side, m_), "dq%s%d" % (side, m_)
+            w("  o[%d * stride] = T(%s * (%s.c[0] + %s.c[3])); o[%d * stride] = T(%s * (%s.c[0] - %s.c[3])); o[%d * stride] = T(%s * %s.c[1]); "
+              "o[%d * stride] = T(%s * %s.c[2]); o[%d * stride] = T(%s * mt_d);\n"
+              % (i, sv, qv, qv, i + 1, sv, qv, qv, i + 2, sv, qv, i + 3, sv, qv, i + 4, sv))
         elif name in ("ub", "vv"):
             fn, mom = ("ext_ubar", "ptd") if name == "ub" else ("ext_v", "ptbd")
             for hi, lam in ((0, "+1"), (8, "-1")):
