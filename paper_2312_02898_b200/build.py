@@ -44,7 +44,7 @@ def generate():
             kw["stage_kb"] = int(os.environ["MG_STAGEKB"])
         if os.environ.get("MG_NOINLINE"):
             kw["noinline"] = os.environ["MG_NOINLINE"] == "1"
-        if os.environ.get("MG_FLAT"):
+        if os.environ.get("MG_FLAT") and n >= 5:
             kw["flat_phase"] = int(os.environ["MG_FLAT"])
         if os.environ.get("MG_LIVEMAX"):
             kw["live_max"] = int(os.environ["MG_LIVEMAX"])

@@ -22,8 +22,13 @@ def choose_kernels(n, max_terms, live_max, acc_max, flat_phase=0):
     phase recomputes the low-multiplicity currents it shares with its neighbours."""
     import os
     flat = int(os.environ.get("MG_FLATPHASE", "0")) or flat_phase
+    if isinstance(flat, dict):
+        flat = dict(flat)
     if flat and os.environ.get("MG_FLAT_LR"):
         flat = {"*": flat, "L": int(os.environ["MG_FLAT_LR"]), "R": int(os.environ["MG_FLAT_LR"])}
+    if flat and os.environ.get("MG_FLAT_T"):
+        flat = dict(flat) if isinstance(flat, dict) else {"*": flat}
+        flat["T"] = int(os.environ["MG_FLAT_T"])
     if flat:
         # every phase its own kernel: short straight-line bodies that stay resident in the instruction caches
         return [[Plan(n, terms=ph, acc_max=acc_max)] for k in partition_terms(n, max_terms=max_terms, max_phase=flat)
@@ -42,8 +47,9 @@ def choose_kernels(n, max_terms, live_max, acc_max, flat_phase=0):
 
 # measured on B200: short kernels win — their straight-line bodies stay in the instruction caches and
 # their live state fits the register file — even though every extra kernel recomputes a few shared currents and
-# adds partial-JAMP slots.  n = 4: 8 kernels of <= 40 terms; n = 5: 80 kernels of <= 24 terms.
-TUNED = {4: dict(max_terms=40, live_max=1000, flat_phase=0), 5: dict(max_terms=170, live_max=12, flat_phase=24)}
+# adds partial-JAMP slots.  n = 4: 8 kernels of <= 40 terms; n = 5: 86 kernels of <= 24 terms (<= 12 for the
+# single-block 5-gluon trees, whose amplitudes touch the most colour flows).
+TUNED = {4: dict(max_terms=40, live_max=1000, flat_phase=0), 5: dict(max_terms=170, live_max=12, flat_phase={"*": 24, "T": 12})}
 
 
 def emit_split(n, block=128, fp32=True, acc_max=6, max_terms=None, sync_every=2, minblocks=2, live_max=None, flat_phase=None, noinline=False,
