@@ -12,6 +12,15 @@
 #pragma once
 #include <cuda_runtime.h>
 
+// Colour-table access: `tab` is an offset into the blocked table.  If the including unit defines MG_CF_CONST (the
+// name of a __constant__ copy of the table, <= 64 KB) the coefficients come through the constant cache with
+// warp-uniform LDC loads; otherwise from the global table `cft` through L1.
+#ifdef MG_CF_CONST
+#define MG_CF_LOAD2(tab, k) make_double2(MG_CF_CONST[(tab) + (k)], MG_CF_CONST[(tab) + (k) + 1])
+#else
+#define MG_CF_LOAD2(tab, k) __ldg(reinterpret_cast<const double2*>(cft + (tab) + (k)))
+#endif
+
 namespace mgc {
 
 template <class T, int NCOL>
@@ -22,7 +31,7 @@ __global__ void __launch_bounds__(128) colour_kernel(const double* __restrict__ 
   if (ievt >= nevt) return;
   const T* __restrict__ jb = jamp + (long long)ih * (2 * NCOL) * stride + ievt;
   T me = T(0);
-  const double* __restrict__ tab = cft;
+  int tab = 0;
 #pragma unroll 1
   for (int i0 = 0; i0 < NCOL; i0 += 8) {
     T zr[8], zi[8];
@@ -31,10 +40,9 @@ __global__ void __launch_bounds__(128) colour_kernel(const double* __restrict__ 
 #pragma unroll 2
     for (int j = i0; j < NCOL; ++j) {
       const T jr = jb[(2 * j) * stride], ji = jb[(2 * j + 1) * stride];
-      const double2* c2 = reinterpret_cast<const double2*>(tab);
 #pragma unroll
       for (int r = 0; r < 4; ++r) {
-        const double2 c = __ldg(c2 + r);
+        const double2 c = MG_CF_LOAD2(tab, 2 * r);
         zr[2 * r] += T(c.x) * jr; zi[2 * r] += T(c.x) * ji;
         zr[2 * r + 1] += T(c.y) * jr; zi[2 * r + 1] += T(c.y) * ji;
       }
@@ -140,17 +148,16 @@ __global__ void __launch_bounds__(PAIRS * GROUPS) gather_colour_kernel(const dou
     if (b >= NB) continue;
     const int i0 = 8 * b;
     // offset of block b in the blocked upper-triangular table: sum_{b' < b} (NCOL - 8 b') * 8
-    const double* __restrict__ tab = cft + (long long)8 * (b * NCOL - 4 * b * (b - 1));
+    int tab = 8 * (b * NCOL - 4 * b * (b - 1));
     T zr[8], zi[8];
 #pragma unroll
     for (int r = 0; r < 8; ++r) { zr[r] = T(0); zi[r] = T(0); }
 #pragma unroll 2
     for (int j = i0; j < NCOL; ++j) {
       const T jr = sJ[(2 * j) * PAIRS + p], ji = sJ[(2 * j + 1) * PAIRS + p];
-      const double2* c2 = reinterpret_cast<const double2*>(tab);
 #pragma unroll
       for (int r = 0; r < 4; ++r) {
-        const double2 c = __ldg(c2 + r);
+        const double2 c = MG_CF_LOAD2(tab, 2 * r);
         zr[2 * r] += T(c.x) * jr; zi[2 * r] += T(c.x) * ji;
         zr[2 * r + 1] += T(c.y) * jr; zi[2 * r + 1] += T(c.y) * ji;
       }

@@ -210,7 +210,6 @@ def _main_unit(E, n, ns, proc, npar, nhel, ncol, ndiag, cfi, cfden, union, inv, 
                            what="invariants kernel, JAMP gather, colour sum (K6), helicity sum (K7), tile loop over the "
                                 "%d diagram-group kernels" % ngroups)]
     w = out.append
-    w('#include "mg_colour.cuh"\n')
     w("// symmetric colour form: me = sum_i J_i^* (CF_ii J_i + 2 sum_{j>i} CF_ij J_j) / %d ; rows blocked by 8\n" % cfden)
     tab = []
     for i0 in range(0, ncol, 8):
@@ -221,6 +220,14 @@ def _main_unit(E, n, ns, proc, npar, nhel, ncol, ndiag, cfi, cfden, union, inv, 
     for k_ in range(0, len(tab), 24):
         w("  " + ", ".join("%d." % v for v in tab[k_:k_ + 24]) + ",\n")
     w("};\n")
+    import os
+    if os.environ.get("MG_CF_CONST") == "1" and len(tab) * 8 <= 62 * 1024:
+        # measured slower (261k vs 271k ME/s, gg->tt~ggg): the 61 KB table thrashes the constant cache; off
+        w("__constant__ double cf_const[%d] = {\n" % len(tab))
+        for k_ in range(0, len(tab), 24):
+            w("  " + ", ".join("%d." % v for v in tab[k_:k_ + 24]) + ",\n")
+        w("};\n#define MG_CF_CONST %s::cf_const\n" % ns)
+    w("}  // namespace\n#include \"mg_colour.cuh\"\nnamespace %s {\n" % ns)
     # gather table (CSR): flow f <- partial slots part_idx[part_ptr[f] .. part_ptr[f+1])
     ptr, idx = [0], []
     for f in range(ncol):
