@@ -152,7 +152,7 @@ __global__ void __launch_bounds__(PAIRS * GROUPS) gather_colour_kernel(const dou
     T zr[8], zi[8];
 #pragma unroll
     for (int r = 0; r < 8; ++r) { zr[r] = T(0); zi[r] = T(0); }
-#pragma unroll 2
+#pragma unroll 4
     for (int j = i0; j < NCOL; ++j) {
       const T jr = sJ[(2 * j) * PAIRS + p], ji = sJ[(2 * j + 1) * PAIRS + p];
 #pragma unroll

@@ -1,14 +1,13 @@
-"""Split kernel shape (n >= 4 gluons): diagram-group kernels + gather + colour + helicity-sum kernels.
+"""Split kernel shape (n >= 4 gluons): invariants + diagram-group + colour + helicity-sum kernels.
 
-Workspace for one tile of E events and one chunk of H helicities (element type T, event index fastest):
-    part[H][NPART][2][E]   partial JAMPs: every diagram group owns a private range of NPART slots (one slot per
-                           colour flow it touches) and writes each exactly once per (event, helicity) — no
-                           read-modify-write, so the group kernels never wait on global loads;
-    jsum[H][NCOL][2][E]    JAMP[f] = sum of the partial slots of flow f (gather kernel, mg_colour.cuh);
+Workspace for one tile of E events and H helicities (element type T, event index fastest):
+    jamp[H][NCOL][2][E]    JAMPs, accumulated in place by the diagram-group kernels: the first kernel (in launch
+                           order) that touches a flow stores, later kernels add with L2 reductions (reduce_mode
+                           "red"; "slots" = the earlier scheme with private partial slots + a gather kernel);
     meh[H][E]              J^dagger CF J per (event, helicity) (colour kernel);
-    inv[NINV][E]           helicity-independent per-event quantities (invariants kernel).
-The launcher loops over event tiles and helicity chunks so that the workspace stays within the size the API
-layer allocated (mg_api.cu: MG5B200_WS_GB).
+    inv[NINV][E]           helicity-independent per-event tables (invariants kernel).
+The launcher loops over event tiles (and helicity chunks if the workspace the API layer allocated is smaller than
+one tile with all helicities: mg_api.cu, MG5B200_WS_GB).
 """
 from math import factorial
 
@@ -228,6 +227,23 @@ def _main_unit(E, n, ns, proc, npar, nhel, ncol, ndiag, cfi, cfden, union, inv, 
             w("  " + ", ".join("%d." % v for v in tab[k_:k_ + 24]) + ",\n")
         w("};\n#define MG_CF_CONST %s::cf_const\n" % ns)
     w("}  // namespace\n#include \"mg_colour.cuh\"\nnamespace %s {\n" % ns)
+    if ncol <= 32 and reduce_mode == "red":
+        # small colour basis: all JAMPs of a (event, helicity) in registers, the symmetric form fully unrolled with the
+        # integer coefficients as immediates — no table loads, every JAMP read once
+        w("#define MG_HAVE_COLOUR_REG 1\n")
+        w("template <class T>\n__global__ void __launch_bounds__(128) colour_reg_kernel(const T* __restrict__ jamp, T* __restrict__ meh,\n"
+          "                                                                    long long stride, long long nevt) {\n")
+        w("  const long long ievt = (long long)blockIdx.x * blockDim.x + threadIdx.x;\n  const int ih = blockIdx.y;\n")
+        w("  if (ievt >= nevt) return;\n")
+        w("  const T* __restrict__ jb = jamp + (long long)ih * (2 * NCOL) * stride + ievt;\n")
+        for f in range(ncol):
+            w("  const T jr%d = jb[%d * stride], ji%d = jb[%d * stride];\n" % (f, 2 * f, f, 2 * f + 1))
+        w("  T me = T(0);\n")
+        for i in range(ncol):
+            zr = " + ".join("T(%d) * jr%d" % (rows[i][j], j) for j in range(i, ncol) if rows[i][j])
+            zi = " + ".join("T(%d) * ji%d" % (rows[i][j], j) for j in range(i, ncol) if rows[i][j])
+            w("  me += jr%d * (%s);\n  me += ji%d * (%s);\n" % (i, zr, i, zi))
+        w("  meh[(long long)ih * stride + ievt] = me;\n}\n")
     # gather table (CSR): flow f <- partial slots part_idx[part_ptr[f] .. part_ptr[f+1])
     ptr, idx = [0], []
     for f in range(ncol):
@@ -319,8 +335,14 @@ static int run(const double* mom, T* me_out, long long nevt, const int* hel_list
       while (hc %% slices) ++slices;          // equal shares (hc is small)
       const int per_thread = (int)(hc / slices);
 %(calls)s
+#ifdef MG_HAVE_COLOUR_REG
+      colour_reg_kernel<T><<<dim3((unsigned)((ne + 127) / 128), (unsigned)hc), 128, 0, st>>>(part, meh, E, ne);
+      mgc::helsum_kernel<T><<<(unsigned)((ne + 255) / 256), 256, 0, st>>>(meh, E, ne, hc, T(norm), me_out + e0,
+          perhel_out ? perhel_out + (long long)h0 * nevt + e0 : (T*)nullptr, nevt, h0 == 0);
+#else
       mgc::gather_colour_sum<T, NCOL>(cft, pptr, pidx, NPART, part, %(jsrc)s, meh, E, ne, hc, T(norm), me_out + e0,
                                       perhel_out ? perhel_out + (long long)h0 * nevt + e0 : (T*)nullptr, nevt, h0 == 0, %(gather)s, st);
+#endif
       nlaunch += %(ngroups)d + %(extra)d;
     }
   }
