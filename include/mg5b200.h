@@ -129,6 +129,11 @@ size_t mg_momenta_bytes(const mg_process_t* p, int64_t nevt);
  * *flops_per_s; synchronises. */
 int mg_fma_peak(int device, int prec, double* flops_per_s);
 
+/* Same for the FP64 tensor cores: sustained rate of mma.sync.m8n8k4.f64 (DMMA.8x8x4, the native FP64 MMA shape of
+ * sm_100a), 8 independent accumulators per warp, 64 warps per SM.  Decides whether the colour contraction (K6) belongs
+ * on the tensor cores.  Returns FLOP/s in *flops_per_s; synchronises. */
+int mg_dmma_peak(int device, double* flops_per_s);
+
 const char* mg_status_string(int status);
 const char* mg_last_error(void); /* thread-local detail of the last MG_ERR_CUDA */
 

@@ -20,7 +20,7 @@ HEL_FILTER, HEL_ALL = 0, 1
 
 SYMBOLS = ["mg_params_default", "mg_process_create", "mg_process_destroy", "mg_rambo", "mg_rambo_ex", "mg_philox_raw", "mg_sigma",
            "mg_sigma_host", "mg_helicity_probe", "mg_sigma_per_helicity", "mg_good_helicities", "mg_process_info",
-           "mg_momenta_bytes", "mg_fma_peak", "mg_status_string", "mg_last_error"]
+           "mg_momenta_bytes", "mg_fma_peak", "mg_dmma_peak", "mg_status_string", "mg_last_error"]
 
 
 class MgParams(C.Structure):
@@ -70,6 +70,7 @@ def lib():
         L.mg_momenta_bytes.argtypes = [vp, i64]
         L.mg_momenta_bytes.restype = C.c_size_t
         L.mg_fma_peak.argtypes = [C.c_int, C.c_int, C.POINTER(C.c_double)]
+        L.mg_dmma_peak.argtypes = [C.c_int, C.POINTER(C.c_double)]
         L.mg_status_string.argtypes = [C.c_int]
         L.mg_status_string.restype = C.c_char_p
         L.mg_last_error.restype = C.c_char_p
@@ -99,6 +100,13 @@ def fma_peak(device=0, precision=FP64):
     """Measured FMA rate (FLOP/s) of the device: the denominator of '% of FP64 peak'."""
     out = C.c_double()
     _check(lib().mg_fma_peak(device, precision, C.byref(out)))
+    return out.value
+
+
+def dmma_peak(device=0):
+    """Measured FP64 tensor-core (DMMA m8n8k4) rate of the device in FLOP/s."""
+    out = C.c_double()
+    _check(lib().mg_dmma_peak(device, C.byref(out)))
     return out.value
 
 

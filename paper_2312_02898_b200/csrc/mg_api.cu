@@ -306,6 +306,15 @@ int mg_fma_peak(int device, int prec, double* flops_per_s) {
   return MG_OK;
 }
 
+int mg_dmma_peak(int device, double* flops_per_s) {
+  if (!flops_per_s) return MG_ERR_NULL;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) { cudaGetLastError(); return MG_ERR_NO_DEVICE; }
+  MG_CUDA(cudaSetDevice(device));
+  MG_CUDA(mg_run_dmma_peak(flops_per_s));
+  return MG_OK;
+}
+
 const char* mg_status_string(int s) {
   switch (s) {
     case MG_OK: return "ok";

@@ -12,5 +12,6 @@ enum { MG_PAR_GS2 = 0, MG_PAR_MT = 1, MG_PAR_E2 = 2, MG_PAR_GL = 3, MG_PAR_GR = 
 cudaError_t mg_launch_rambo(int nfinal, const double* masses, double sqrt_s, uint64_t seed, long long first_event,
                             long long nevt, double* mom, double* wgt, cudaStream_t st);
 cudaError_t mg_run_fma_peak(int prec, double* flops_per_s);
+cudaError_t mg_run_dmma_peak(double* flops_per_s);
 cudaError_t mg_launch_philox_raw(uint64_t seed, long long first_event, long long nevt, int nfinal, uint32_t* out,
                                  cudaStream_t st);

@@ -53,6 +53,57 @@ template <class T> cudaError_t run(double* flops_per_s) {
 }
 }  // namespace
 
+namespace {
+// FP64 tensor-core rate: mma.sync.m8n8k4.f64 (DMMA.8x8x4), 8 independent accumulator pairs per warp
+__global__ void __launch_bounds__(256) dmma_peak_kernel(double* out, int iters, double a, double b) {
+  double c0[8], c1[8];
+#pragma unroll
+  for (int k = 0; k < 8; ++k) { c0[k] = threadIdx.x * 1e-3 + k; c1[k] = -c0[k]; }
+#pragma unroll 1
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int r = 0; r < 4; ++r) {
+#pragma unroll
+      for (int k = 0; k < 8; ++k)
+        asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                     : "+d"(c0[k]), "+d"(c1[k]) : "d"(a), "d"(b));
+    }
+  }
+  double s = 0;
+#pragma unroll
+  for (int k = 0; k < 8; ++k) s += c0[k] + c1[k];
+  if (s == -1.2345) out[blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+}  // namespace
+
+cudaError_t mg_run_dmma_peak(double* flops_per_s) {
+  int dev = 0, nsm = 0;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
+  const int block = 256, grid = nsm * 8, iters = 2000;
+  double* out = nullptr;
+  cudaError_t e = cudaMalloc(&out, sizeof(double) * (size_t)block * grid);
+  if (e != cudaSuccess) return e;
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0); cudaEventCreate(&e1);
+  double best = 0;
+  for (int rep = 0; rep < 5; ++rep) {
+    cudaEventRecord(e0);
+    dmma_peak_kernel<<<grid, block>>>(out, iters, 1e-3, 1e-3);
+    cudaEventRecord(e1);
+    e = cudaEventSynchronize(e1);
+    if (e != cudaSuccess) break;
+    float ms = 0;
+    cudaEventElapsedTime(&ms, e0, e1);
+    const double fl = 2.0 * 8 * 8 * 4 * 8 * 4 * (double)iters * (block / 32) * (double)grid;   // 512 flop per mma per warp
+    if (rep >= 1 && fl / (ms * 1e-3) > best) best = fl / (ms * 1e-3);
+  }
+  cudaEventDestroy(e0); cudaEventDestroy(e1);
+  cudaFree(out);
+  *flops_per_s = best;
+  return e != cudaSuccess ? e : cudaGetLastError();
+}
+
 cudaError_t mg_run_fma_peak(int prec, double* flops_per_s) {
   return prec == 0 ? run<double>(flops_per_s) : run<float>(flops_per_s);
 }

@@ -226,6 +226,11 @@ def _main_unit(E, n, ns, proc, npar, nhel, ncol, ndiag, cfi, cfden, union, inv, 
         for k_ in range(0, len(tab), 24):
             w("  " + ", ".join("%d." % v for v in tab[k_:k_ + 24]) + ",\n")
         w("};\n#define MG_CF_CONST %s::cf_const\n" % ns)
+    # dense table for the DMMA variant of the colour sum (CF integers; the denominator is folded into `norm`)
+    w("__device__ __align__(16) const double cf_dense[%d] = {\n" % (ncol * ncol))
+    for i in range(ncol):
+        w("  " + ", ".join("%d." % cfi[i][j] for j in range(ncol)) + ",\n")
+    w("};\n")
     w("}  // namespace\n#include \"mg_colour.cuh\"\nnamespace %s {\n" % ns)
     if ncol <= 32 and reduce_mode == "red":
         # small colour basis: all JAMPs of a (event, helicity) in registers, the symmetric form fully unrolled with the
@@ -314,6 +319,8 @@ static int run(const double* mom, T* me_out, long long nevt, const int* hel_list
   if (H > 8) H = H / 4 * 4;
   const double* cft = nullptr; const short* pptr = nullptr; const short* pidx = nullptr;
   cudaGetSymbolAddress((void**)&cft, cf_table);
+  const double* cfd = nullptr;
+  cudaGetSymbolAddress((void**)&cfd, cf_dense);
   cudaGetSymbolAddress((void**)&pptr, part_ptr);
   cudaGetSymbolAddress((void**)&pidx, part_idx);
   T* part = (T*)ws;
@@ -341,7 +348,7 @@ static int run(const double* mom, T* me_out, long long nevt, const int* hel_list
           perhel_out ? perhel_out + (long long)h0 * nevt + e0 : (T*)nullptr, nevt, h0 == 0);
 #else
       mgc::gather_colour_sum<T, NCOL>(cft, pptr, pidx, NPART, part, %(jsrc)s, meh, E, ne, hc, T(norm), me_out + e0,
-                                      perhel_out ? perhel_out + (long long)h0 * nevt + e0 : (T*)nullptr, nevt, h0 == 0, %(gather)s, st);
+                                      perhel_out ? perhel_out + (long long)h0 * nevt + e0 : (T*)nullptr, nevt, h0 == 0, %(gather)s, st, cfd);
 #endif
       nlaunch += %(ngroups)d + %(extra)d;
     }

@@ -268,3 +268,6 @@ def test_fma_peak_is_plausible(mg):
     p64 = mg.fma_peak(0, mg.FP64)
     p32 = mg.fma_peak(0, mg.FP32)
     assert 5e12 < p64 < 1e14 and 2e13 < p32 < 2e14
+    pd = mg.dmma_peak(0)
+    assert 1e11 < pd < 2e14
+    print("measured peaks: DFMA %.2f, FFMA %.2f, DMMA %.2f TFLOP/s" % (p64 / 1e12, p32 / 1e12, pd / 1e12))
