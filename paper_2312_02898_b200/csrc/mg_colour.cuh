@@ -184,7 +184,7 @@ __global__ void __launch_bounds__(PAIRS * GROUPS) gather_colour_kernel(const dou
 // CTA = 4 warps x 32 events of one helicity; the 2*NCOL x 32 JAMP tile is staged once in shared memory (B operand:
 // k = flow j, n = (event, re/im)); warp w owns the row blocks w, w+4, ... of CF (A operand, dense [NCOL][NCOL]
 // table in global memory, L1-resident) and reuses every A fragment for the 8 column tiles.  The dense product
-// costs twice the FLOPs of the symmetric register-blocked form at the same peak rate.
+// uses the symmetry of CF at the level of 8x8 blocks (upper block triangle only, off-diagonal blocks doubled).
 template <int NCOL>
 __global__ void __launch_bounds__(128) colour_dmma_kernel(const double* __restrict__ cfd, const double* __restrict__ jamp,
                                                           double* __restrict__ meh, long long stride, long long nevt) {
@@ -208,13 +208,18 @@ __global__ void __launch_bounds__(128) colour_dmma_kernel(const double* __restri
   double mep[8];
 #pragma unroll
   for (int ct = 0; ct < 8; ++ct) mep[ct] = 0.0;
-  for (int rb = w; rb < NCOL / 8; rb += 4) {
+  // block-triangular: row block rb only meets column blocks kb >= rb (the table holds CF on the diagonal blocks and
+  // 2 CF above them), which halves the MMAs; warps take row blocks boustrophedon to balance the triangle
+  for (int t = 0;; ++t) {
+    const int rb = (t & 1) ? (t + 1) * 4 - 1 - w : t * 4 + w;
+    if (t * 4 >= NCOL / 8) break;
+    if (rb >= NCOL / 8) continue;
     double c0[8], c1[8];
 #pragma unroll
     for (int ct = 0; ct < 8; ++ct) { c0[ct] = 0.0; c1[ct] = 0.0; }
     const double* __restrict__ arow = cfd + (long long)(rb * 8 + ar) * NCOL + ak;
 #pragma unroll 2
-    for (int k0 = 0; k0 < NCOL; k0 += 4) {
+    for (int k0 = rb * 8; k0 < NCOL; k0 += 4) {
       const double a = __ldg(arow + k0);
       const double* __restrict__ brow = sJ + (2 * (k0 + ak) + bc) * RS + bp;
 #pragma unroll

@@ -228,8 +228,9 @@ def _main_unit(E, n, ns, proc, npar, nhel, ncol, ndiag, cfi, cfden, union, inv, 
         w("};\n#define MG_CF_CONST %s::cf_const\n" % ns)
     # dense table for the DMMA variant of the colour sum (CF integers; the denominator is folded into `norm`)
     w("__device__ __align__(16) const double cf_dense[%d] = {\n" % (ncol * ncol))
-    for i in range(ncol):
-        w("  " + ", ".join("%d." % cfi[i][j] for j in range(ncol)) + ",\n")
+    for i in range(ncol):      # diagonal 8x8 blocks: CF; blocks above: 2 CF; blocks below: unused (0)
+        w("  " + ", ".join("%d." % (cfi[i][j] if j // 8 == i // 8 else 2 * cfi[i][j] if j // 8 > i // 8 else 0)
+                           for j in range(ncol)) + ",\n")
     w("};\n")
     w("}  // namespace\n#include \"mg_colour.cuh\"\nnamespace %s {\n" % ns)
     if ncol <= 32 and reduce_mode == "red":
