@@ -108,8 +108,9 @@ int mg_philox_raw(mg_process_t* p, uint64_t seed, int64_t first_event, int64_t n
  * the first call that needs a bigger one. */
 int mg_sigma(mg_process_t* p, const void* momenta_dev, int64_t nevt, void* me_out_dev, void* stream);
 
-/* Same from HOST buffers (momenta_host: layout above, me_out_host: nevt elements): copies in, runs, copies
- * out and synchronises.  This is the end-to-end entry point bench.py times as `e2e`. */
+/* Same from HOST buffers (momenta_host: layout above, me_out_host: nevt elements; pinned memory recommended): copies
+ * in, runs, copies out and synchronises.  The device staging buffers belong to the handle, grow on demand and are
+ * freed by mg_process_destroy.  This is the end-to-end entry point bench.py times as `e2e`. */
 int mg_sigma_host(mg_process_t* p, const void* momenta_host, int64_t nevt, void* me_out_host, void* stream);
 
 /* K8: explicit helicity probe on nprobe events; sets the good-helicity list (synchronises). */

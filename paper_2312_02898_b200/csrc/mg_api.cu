@@ -33,6 +33,8 @@ struct mg_process {
   std::vector<int> good;
   bool probed;
   long long launches;      // kernels launched by the last mg_sigma / mg_sigma_per_helicity call
+  void* io_mom; size_t io_mom_bytes;   // device staging of mg_sigma_host (grow-only, library-owned)
+  void* io_out; size_t io_out_bytes;
   void* ws;                // workspace of the split kernel shape (JAMPs + per-helicity values), library-owned
   size_t ws_bytes;
 };
@@ -105,6 +107,7 @@ int mg_process_create(const char* proc, const mg_params_t* params, mg_process_t*
   MG_CUDA(cudaSetDevice(params->device));
   mg_process* p = new mg_process();
   p->desc = d; p->par = *params; p->probed = false; p->ws = nullptr; p->ws_bytes = 0; p->launches = 0;
+  p->io_mom = p->io_out = nullptr; p->io_mom_bytes = p->io_out_bytes = 0;
   p->nfinal = d->npar - 2;
   for (int i = 0; i < 8; ++i) p->masses[i] = (i < d->npar && d->massive[i]) ? params->mt : 0.0;
   // derived couplings (DESIGN.md §3 C2, reading A1)
@@ -145,6 +148,8 @@ int mg_process_destroy(mg_process_t* p) {
   cudaFree(p->hel_dev);
   cudaFree(p->hel_all_dev);
   if (p->ws) cudaFree(p->ws);
+  if (p->io_mom) cudaFree(p->io_mom);
+  if (p->io_out) cudaFree(p->io_out);
   delete p;
   return MG_OK;
 }
@@ -256,17 +261,24 @@ int mg_sigma_host(mg_process_t* p, const void* momenta_host, int64_t nevt, void*
   if (nevt == 0) return MG_OK;
   MG_CUDA(cudaSetDevice(p->par.device));
   cudaStream_t st = (cudaStream_t)stream;
-  void *dm = nullptr, *dout = nullptr;
-  const size_t mb = mg_momenta_bytes(p, nevt);
-  MG_CUDA(cudaMallocAsync(&dm, mb, st));
-  cudaError_t e = cudaMallocAsync(&dout, esize(p) * (size_t)nevt, st);
-  if (e != cudaSuccess) { cudaFreeAsync(dm, st); return cuda_fail(e, "cudaMallocAsync"); }
+  // device staging buffers are kept in the handle and only ever grow (a stream-ordered allocation per call showed
+  // occasional second-long stalls when the pool returned memory to the OS between calls)
+  const size_t mb = mg_momenta_bytes(p, nevt), ob = esize(p) * (size_t)nevt;
+  if (p->io_mom_bytes < mb) {
+    if (p->io_mom) { cudaDeviceSynchronize(); cudaFree(p->io_mom); p->io_mom = nullptr; p->io_mom_bytes = 0; }
+    MG_CUDA(cudaMalloc(&p->io_mom, mb));
+    p->io_mom_bytes = mb;
+  }
+  if (p->io_out_bytes < ob) {
+    if (p->io_out) { cudaDeviceSynchronize(); cudaFree(p->io_out); p->io_out = nullptr; p->io_out_bytes = 0; }
+    MG_CUDA(cudaMalloc(&p->io_out, ob));
+    p->io_out_bytes = ob;
+  }
+  void *dm = p->io_mom, *dout = p->io_out;
   int rc = MG_OK;
-  e = cudaMemcpyAsync(dm, momenta_host, mb, cudaMemcpyHostToDevice, st);
+  cudaError_t e = cudaMemcpyAsync(dm, momenta_host, mb, cudaMemcpyHostToDevice, st);
   if (e == cudaSuccess) rc = mg_sigma(p, dm, nevt, dout, stream);
-  if (e == cudaSuccess && rc == MG_OK) e = cudaMemcpyAsync(me_out_host, dout, esize(p) * (size_t)nevt, cudaMemcpyDeviceToHost, st);
-  cudaFreeAsync(dm, st);
-  cudaFreeAsync(dout, st);
+  if (e == cudaSuccess && rc == MG_OK) e = cudaMemcpyAsync(me_out_host, dout, ob, cudaMemcpyDeviceToHost, st);
   cudaError_t es = cudaStreamSynchronize(st);
   if (rc != MG_OK) return rc;
   if (e != cudaSuccess) return cuda_fail(e, "mg_sigma_host copy");
