@@ -56,8 +56,8 @@ static int ensure_ws(mg_process* p, int64_t nevt, int nhel_run) {
   if (const char* e = getenv("MG5B200_WS_GB")) { const double v = atof(e); if (v > 0) cap_gb = v; }
   const size_t cap = (size_t)(cap_gb * 1073741824.0);
   size_t E = (size_t)((nevt + 31) / 32 * 32);
-  if (E > 131072) E = 131072;
-  size_t need = E * (per_e + (size_t)nhel_run * per_eh);      // whole helicity list resident
+  if (E > ((size_t)1 << 20)) E = (size_t)1 << 20;             // the launcher's largest event tile
+  size_t need = E * (per_e + (size_t)nhel_run * per_eh);      // whole batch, whole helicity list resident
   if (need > cap) need = cap;
   const size_t floor_bytes = (E < 1024 ? E : 1024) * (per_e + 4 * per_eh);
   if (need < floor_bytes) need = floor_bytes;

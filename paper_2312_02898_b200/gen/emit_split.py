@@ -300,6 +300,9 @@ def _main_unit(E, n, ns, proc, npar, nhel, ncol, ndiag, cfi, cfden, union, inv, 
             w("  stp(o + %d * stride, stride, %s);\n" % (i, name))
     w("}\n")
     w("""
+#ifndef MG_TILE_MAX
+#define MG_TILE_MAX (1 << 20)
+#endif
 template <class T>
 static int run(const double* mom, T* me_out, long long nevt, const int* hel_list, int nhel_run, T* perhel_out,
                 const double* par, void* ws, size_t ws_bytes, cudaStream_t st, int prec) {
@@ -309,15 +312,22 @@ static int run(const double* mom, T* me_out, long long nevt, const int* hel_list
   const size_t es = sizeof(T);
   const size_t per_eh = (size_t)(%(slots)s + 2 * NCOL + 1) * es;     // bytes per (event, helicity)
   const size_t per_e = (size_t)NINV * es;                            // bytes per event
-  // event tile E (multiple of 1024, or the whole padded batch) and helicity chunk H
+  // Event tile E and helicity chunk H.  Prefer the whole batch in one tile (one launch per kernel covers many waves
+  // of CTAs: with 2 CTAs of 128 threads per SM a 131072-event tile is 3.46 waves, i.e. the last wave is half empty)
+  // and chunk the helicities if the workspace is too small; only shrink the tile when fewer than MINH helicities fit.
+  const long long EMAX = (long long)MG_TILE_MAX;
   long long E = (nevt + 31) / 32 * 32;
-  if (E > 131072) E = 131072;
-  while (E > 1024 && (size_t)E * (per_e + 4 * per_eh) > ws_bytes) E = (E / 2 + 1023) / 1024 * 1024;
+  if (E > EMAX) E = EMAX;
+  const long long MINH = nhel_run < 16 ? nhel_run : 16;
+  while (E > 1024 && (size_t)E * (per_e + MINH * per_eh) > ws_bytes) E = (E / 2 + 1023) / 1024 * 1024;
   if ((size_t)E * (per_e + per_eh) > ws_bytes) return 0;            // mg_api.cu sizes the workspace; cannot happen
   int nlaunch = 0;
   long long H = (long long)((ws_bytes / (size_t)E - per_e) / per_eh);
   if (H > nhel_run) H = nhel_run;
-  if (H > 8) H = H / 4 * 4;
+  if (H < nhel_run) {                                               // equal chunks
+    const long long nchunk = (nhel_run + H - 1) / H;
+    H = (nhel_run + nchunk - 1) / nchunk;
+  }
   const double* cft = nullptr; const short* pptr = nullptr; const short* pidx = nullptr;
   cudaGetSymbolAddress((void**)&cft, cf_table);
   const double* cfd = nullptr;
@@ -340,7 +350,7 @@ static int run(const double* mom, T* me_out, long long nevt, const int* hel_list
       long long slices = (148LL * 256 * 3 + ne - 1) / ne;
       if (slices > hc) slices = hc;
       if (slices < 1) slices = 1;
-      while (hc %% slices) ++slices;          // equal shares (hc is small)
+      while (hc %% slices) ++slices;          // equal shares
       const int per_thread = (int)(hc / slices);
 %(calls)s
 #ifdef MG_HAVE_COLOUR_REG
