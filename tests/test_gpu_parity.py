@@ -264,6 +264,30 @@ def test_edge_cases_and_errors(mg, oracle_ld):
     assert np.allclose(proc2.sigma(mom, 100).cpu().numpy(), me[:100] * 8.0, rtol=1e-12)
 
 
+@pytest.mark.parametrize("name,nevt,ws_gb", [("ggttgg", 20011, 0.05), ("ggttgg", 20011, 0.004), ("ggttggg", 3001, 0.05)])
+def test_small_workspace_tiles_and_helicity_chunks_give_identical_results(mg, name, nevt, ws_gb):
+    """The launcher falls back to helicity chunks and smaller event tiles when the workspace cap (MG5B200_WS_GB) is
+    low.  Event tiles do not change any per-event arithmetic; helicity chunks change only the association of the final
+    helicity sum (chunk sums are added one after the other), so the results agree to rounding (1e-14)."""
+    import os
+    import torch
+    cfg = workloads.CONFIGS[name]
+    ref_proc = mg.Process(cfg["proc"])
+    mom = ref_proc.rambo(cfg["seed"], cfg["sqrt_s"], nevt)
+    ref = ref_proc.sigma(mom, nevt).cpu().numpy()
+    big_ws = ref_proc.info.workspace_bytes
+    os.environ["MG5B200_WS_GB"] = repr(ws_gb)
+    try:
+        proc = mg.Process(cfg["proc"])
+        proc.helicity_probe(mom, min(nevt, 4096))
+        got = proc.sigma(mom, nevt).cpu().numpy()
+        assert 0 < proc.info.workspace_bytes < big_ws
+        assert proc.info.launches_last_sigma > ref_proc.info.launches_last_sigma
+    finally:
+        del os.environ["MG5B200_WS_GB"]
+    assert np.max(np.abs(got / ref - 1)) < 1e-14
+
+
 def test_fma_peak_is_plausible(mg):
     p64 = mg.fma_peak(0, mg.FP64)
     p32 = mg.fma_peak(0, mg.FP32)
