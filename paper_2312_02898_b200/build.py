@@ -38,6 +38,8 @@ def generate():
             kw["block"] = int(block[str(n)])
         if str(n) in maxterms:
             kw["max_terms"] = int(maxterms[str(n)])
+        if os.environ.get("MG_PREFETCH"):
+            kw["prefetch"] = int(os.environ["MG_PREFETCH"])
         if os.environ.get("MG_REDUCE"):
             kw["reduce_mode"] = os.environ["MG_REDUCE"]
         if os.environ.get("MG_STAGEKB"):

@@ -48,16 +48,18 @@ def choose_kernels(n, max_terms, live_max, acc_max, flat_phase=0):
 # their live state fits the register file — even though every extra kernel recomputes a few shared currents and
 # adds partial-JAMP slots.  n = 4: 8 kernels of <= 40 terms; n = 5: 86 kernels of <= 24 terms (<= 12 for the
 # single-block 5-gluon trees, whose amplitudes touch the most colour flows).
-TUNED = {4: dict(max_terms=40, live_max=1000, flat_phase=0), 5: dict(max_terms=170, live_max=12, flat_phase={"*": 24, "T": 12})}
+TUNED = {4: dict(max_terms=40, live_max=1000, flat_phase=0, prefetch=0),
+         5: dict(max_terms=170, live_max=12, flat_phase={"*": 24, "T": 12}, prefetch=1)}
 
 
 def emit_split(n, block=128, fp32=True, acc_max=6, max_terms=None, sync_every=2, minblocks=2, live_max=None, flat_phase=None, noinline=False,
-               stage_kb=110, reduce_mode="red"):
+               stage_kb=110, reduce_mode="red", prefetch=None):
     from . import emit as E
     tuned = TUNED.get(n, TUNED[5])
     max_terms = max_terms or tuned["max_terms"]
     live_max = live_max or tuned["live_max"]
     flat_phase = tuned["flat_phase"] if flat_phase is None else flat_phase
+    prefetch = tuned["prefetch"] if prefetch is None else prefetch      # n = 5: +1.2 %; n = 4: -1.5 % (measured)
     kernels = choose_kernels(n, max_terms, live_max, acc_max, flat_phase)
     npar, nhel = n + 2, 1 << (n + 2)
     ns = "mg_ggtt" + "g" * (n - 2)
@@ -146,7 +148,7 @@ def emit_split(n, block=128, fp32=True, acc_max=6, max_terms=None, sync_every=2,
 
         for pi, plan in enumerate(phases):
             w("    {   // phase %d: %d terms, <= %d live currents\n" % (pi, len(plan.terms), plan.max_live()))
-            E._body(plan, w, sink, acc, sync_every=sync_every, noinline=noinline)
+            E._body(plan, w, sink, acc, sync_every=sync_every, noinline=noinline, prefetch=prefetch)
             w("    }\n")
         w("    if (live) {\n")
         if reduce_mode == "red":
