@@ -33,7 +33,9 @@ def generate():
     block = dict(kv.split("=") for kv in os.environ.get("MG_BLOCK", "").split(",") if kv)
     jobs = [emit_eemumu()]
     for n in ns_gluons:
-        kw = dict(fp32=(n < 5), acc_max=int(os.environ.get("MG_ACCMAX", "6")))
+        kw = dict(fp32=(n < 5))
+        if os.environ.get("MG_ACCMAX"):
+            kw["acc_max"] = int(os.environ["MG_ACCMAX"])
         if str(n) in block:
             kw["block"] = int(block[str(n)])
         if str(n) in maxterms:

@@ -52,7 +52,7 @@ TUNED = {4: dict(max_terms=40, live_max=1000, flat_phase=0, prefetch=0),
          5: dict(max_terms=170, live_max=12, flat_phase={"*": 24, "T": 12}, prefetch=1)}
 
 
-def emit_split(n, block=128, fp32=True, acc_max=6, max_terms=None, sync_every=2, minblocks=2, live_max=None, flat_phase=None, noinline=False,
+def emit_split(n, block=128, fp32=True, acc_max=24, max_terms=None, sync_every=2, minblocks=2, live_max=None, flat_phase=None, noinline=False,
                stage_kb=110, reduce_mode="red", prefetch=None):
     from . import emit as E
     tuned = TUNED.get(n, TUNED[5])
@@ -377,7 +377,7 @@ static int launch(int prec, const double* mom, void* me_out, long long nevt, con
 }  // namespace
 extern const mg_procdesc_t mg_desc_%(tag)s = {"%(proc)s", %(npar)d, %(nfinal)d, %(ndiag)d, %(nhel)d, %(ncol)d, %(denom)d,
   %(flops)dLL, {0, 0, 1, 1%(gm)s}, %(ns)s::launch, {%(ws64)d, %(ws32)d}, %(nk)d, %(hasfp32)d, {%(wse64)d, %(wse32)d}, %(algo)dLL};
-""" % dict(ngroups=ngroups, algo=Plan(n, acc_max=6).flops_per_helicity(externals=False), cfden=cfden, denom=denom, tag=ns[3:], proc=proc, npar=npar, nfinal=n, ndiag=ndiag, nhel=nhel, ncol=ncol,
+""" % dict(ngroups=ngroups, algo=Plan(n, acc_max=24).flops_per_helicity(externals=False), cfden=cfden, denom=denom, tag=ns[3:], proc=proc, npar=npar, nfinal=n, ndiag=ndiag, nhel=nhel, ncol=ncol,
            flops=group_flops + colour_flops, gm=", 0" * (n - 2), ns=ns,
            ws64=((0 if reduce_mode == "red" else 2 * npart) + 2 * ncol + 1) * 8,
            ws32=((0 if reduce_mode == "red" else 2 * npart) + 2 * ncol + 1) * 4,
