@@ -461,7 +461,7 @@ def group_key(term, n):
     if th <= len(la) < n:
         return ("A", tuple(sorted(la))), big_child(anc)
     if len(la) >= n:
-        return ("T", mid[0]), big_child(mid)
+        return ("T", "all"), (mid[0], big_child(mid))      # one coarse class: every T kernel touches most flows
     # quark-line dominated terms: keyed by the gluon *set* on the top side of the closing block (the terms of a set
     # share all their top-side chains and need antitop-side chains over the complement only), then by the closing
     # block; terms closed on their first block are keyed by that block
