@@ -101,7 +101,7 @@ def run_reference(args, name, cfg):
 
 # DRAM bytes (read + write) moved by all kernels of one mg_sigma call at the full batch size, from ncu captures
 # (dram__bytes_read.sum + dram__bytes_write.sum summed over the launches of one call); see the named file.
-DRAM_TRAFFIC = {("ggttgg", "fp64"): (190e9, "profiles/r1_launches_ggttgg.md"),
+DRAM_TRAFFIC = {("ggttgg", "fp64"): (157e9, "profiles/r1_launches_ggttgg.md"),
                 ("ggttggg", "fp64"): (2767e9, "profiles/r1_launches_ggttggg.md")}
 
 

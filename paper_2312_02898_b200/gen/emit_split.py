@@ -25,6 +25,9 @@ def choose_kernels(n, max_terms, live_max, acc_max, flat_phase=0):
         flat = dict(flat)
     if flat and os.environ.get("MG_FLAT_LR"):
         flat = {"*": flat, "L": int(os.environ["MG_FLAT_LR"]), "R": int(os.environ["MG_FLAT_LR"])}
+    if flat and os.environ.get("MG_FLAT_A"):
+        flat = dict(flat) if isinstance(flat, dict) else {"*": flat}
+        flat["A"] = int(os.environ["MG_FLAT_A"])
     if flat and os.environ.get("MG_FLAT_T"):
         flat = dict(flat) if isinstance(flat, dict) else {"*": flat}
         flat["T"] = int(os.environ["MG_FLAT_T"])
