@@ -49,7 +49,7 @@ def choose_kernels(n, max_terms, live_max, acc_max, flat_phase=0):
 
 # measured on B200: short kernels win — their straight-line bodies stay in the instruction caches and
 # their live state fits the register file — even though every extra kernel recomputes a few shared currents and
-# adds partial-JAMP slots.  n = 4: 8 kernels of <= 40 terms; n = 5: 86 kernels of <= 24 terms (<= 12 for the
+# adds partial-JAMP slots.  n = 4: 7 kernels of <= 40 terms; n = 5: 86 kernels of <= 24 terms (<= 12 for the
 # single-block 5-gluon trees, whose amplitudes touch the most colour flows).
 TUNED = {4: dict(max_terms=40, live_max=1000, flat_phase=0, prefetch=0),
          5: dict(max_terms=170, live_max=12, flat_phase={"*": 24, "T": 12}, prefetch=1)}
