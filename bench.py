@@ -8,8 +8,8 @@ mg_rambo (device Philox + RAMBO) followed by mg_sigma on BASELINE.json's configu
 g g > t t~ g g, 524288 events, sqrt(s) = 1500 GeV, seed 4, fp64 — the first process BASELINE.json's metric
 is quoted on).  Prints ONE JSON line (contract in the task statement): `value` = ME/s with inputs resident
 in HBM; `e2e` = the same through mg_sigma_host with pinned HOST buffers (H2D/D2H inside the timed region);
-`roofline` = achieved FP64 FLOP/s of the sigma kernel(s) against the FMA peak measured in the same run
-(mg_fma_peak), bound "alu"; `cpu_baseline` = the CPU oracle timed on this box's host cores on a bounded
+`roofline` = achieved FP64 FLOP/s of the sigma kernel(s) against the larger of the nominal DFMA peak and the FMA-loop
+rate measured in the same run (libmg5b200_peak.so), bound "alu"; `cpu_baseline` = the CPU oracle timed on this box's host cores on a bounded
 sample.  `--impl reference` times the oracle alone (it is the reference arm of this tier).
 Under torchrun each rank takes its own shard of the Philox event stream (first_event = rank * nevt): weak
 scaling, no data-path collective.
@@ -35,11 +35,12 @@ def parse():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--workload", default=os.environ.get("MG_BENCH_WORKLOAD", "ggttgg"), choices=list(workloads.CONFIGS))
+    ap.add_argument("--workload", default="ggttgg", choices=list(workloads.CONFIGS))
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--precision", default="fp64", choices=["fp64", "fp32"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--nevt", type=int, default=0, help="override the batch size (profiling runs only; not a bench value)")
+    ap.add_argument("--single", action="store_true", help="only the named workload (no second process under 'also')")
     return ap.parse_args()
 
 
@@ -99,10 +100,31 @@ def run_reference(args, name, cfg):
     return 0
 
 
-# DRAM bytes (read + write) moved by all kernels of one mg_sigma call at the full batch size, from ncu captures
-# (dram__bytes_read.sum + dram__bytes_write.sum summed over the launches of one call); see the named file.
-DRAM_TRAFFIC = {("ggttgg", "fp64"): (157e9, "profiles/r1_launches_ggttgg.md"),
-                ("ggttggg", "fp64"): (2767e9, "profiles/r1_launches_ggttggg.md")}
+def dram_traffic(name, precision):
+    """DRAM bytes (read + write) moved by all kernels of one mg_sigma call at the full batch size, from the ncu capture
+    summarised in profiles/r2_traffic.csv (columns: workload, precision, bytes_per_call, source); None if absent."""
+    path = os.path.join(ROOT, "profiles", "r2_traffic.csv")
+    if not os.path.exists(path):
+        return None
+    for line in open(path):
+        f = [x.strip() for x in line.split(",")]
+        if len(f) >= 4 and f[0] == name and f[1] == precision:
+            return float(f[2]), f[3]
+    return None
+
+
+def measured_peaks(device):
+    """DFMA / FFMA / DMMA rates of the device measured now with the helper library libmg5b200_peak.so (FLOP/s)."""
+    import ctypes as C
+    L = C.CDLL(os.path.join(ROOT, "paper_2312_02898_b200", "libmg5b200_peak.so"))
+    out = {}
+    v = C.c_double()
+    for key, prec in (("dfma", 0), ("ffma", 1)):
+        assert L.mgpeak_fma(device, prec, C.byref(v)) == 0
+        out[key] = v.value
+    assert L.mgpeak_dmma(device, C.byref(v)) == 0
+    out["dmma"] = v.value
+    return out
 
 
 # ---------------------------------------------------------------------------------------------- clocks
@@ -151,6 +173,123 @@ class ClockSampler:
 
 
 # ---------------------------------------------------------------------------------------------- main arm
+NOMINAL_FP64 = 148 * 64 * 2 * 1.965e9        # B200: 148 SMs x 64 FP64 lanes x 2 (FMA) x 1.965 GHz = 37.2 TFLOP/s
+NOMINAL_FP32 = 148 * 128 * 2 * 1.965e9
+
+
+def measure(mg, torch, dist, name, cfg, args, steps, rank, world, local, peaks, with_clocks):
+    """Times `steps` steps of workload `name` (after >= 3 warm-ups); returns the fields of the JSON line."""
+    prec = mg.FP64 if args.precision == "fp64" else mg.FP32
+    proc = mg.Process(cfg["proc"], precision=prec, device=local)
+    nevt = cfg["nevt"]
+    first, _ = mg.shard(nevt, rank, world)
+    st = torch.cuda.current_stream()
+    mom = proc.alloc_momenta(nevt)
+    me = torch.empty(nevt, dtype=torch.float64 if prec == mg.FP64 else torch.float32, device=mom.device)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=mom.device)
+    # set-up outside the timed region: helicity probe (K8)
+    proc.rambo(cfg["seed"], cfg["sqrt_s"], nevt, first_event=first, out=mom)
+    proc.helicity_probe(mom, min(nevt, 4096))
+
+    def step(ev=None):
+        if ev:
+            ev[0].record(st)
+        proc.rambo(cfg["seed"], cfg["sqrt_s"], nevt, first_event=first, out=mom, stream=st)
+        if ev:
+            ev[1].record(st)
+        proc.sigma(mom, nevt, out=me, stream=st)
+        if ev:
+            ev[2].record(st)
+
+    warm = max(args.warmup, 3)
+    for _ in range(warm):
+        step()
+    torch.cuda.synchronize()
+    sampler = ClockSampler(local)
+    if rank == 0 and with_clocks:
+        sampler.start()
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(steps)]
+    if dist:
+        dist.barrier()
+    torch.cuda.synchronize()
+    for k in range(steps):
+        flush.fill_(k & 0xFF)             # L2 flush between timed steps (not timed)
+        step(evs[k])
+    torch.cuda.synchronize()
+    if dist:
+        dist.barrier()
+    t_rambo = sum(e[0].elapsed_time(e[1]) for e in evs) * 1e-3
+    t_sigma = sum(e[1].elapsed_time(e[2]) for e in evs) * 1e-3
+    t_total = t_rambo + t_sigma
+
+    # e2e: host buffers through the C ABI (mg_sigma_host): H2D of the momenta + D2H of |M|^2 in the timed region
+    host_mom = torch.empty(mom.numel(), dtype=torch.float64).pin_memory()
+    host_mom.copy_(mom)
+    host_me = torch.empty(nevt, dtype=me.dtype).pin_memory()
+    ne2e = max(3, min(steps, 5))
+    proc.sigma_host(host_mom, nevt, out_host=host_me)
+    torch.cuda.synchronize()
+    if dist:
+        dist.barrier()
+    t0 = time.perf_counter()
+    for _ in range(ne2e):
+        proc.sigma_host(host_mom, nevt, out_host=host_me)      # synchronises internally
+    t_e2e = (time.perf_counter() - t0) / ne2e
+    clocks = sampler.stop() if (rank == 0 and with_clocks) else None
+    assert torch.equal(host_me.cuda(), me), "host and device entry points disagree"
+
+    if dist:
+        t = torch.tensor([t_total, t_sigma, t_rambo, t_e2e], dtype=torch.float64, device=mom.device)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        t_total, t_sigma, t_rambo, t_e2e = [float(x) for x in t]
+    info = proc.info
+    launches_per_step = int(info.launches_last_sigma) + 1            # the sigma kernels + the RAMBO kernel
+    flops_call = float(info.flops_per_event_goodhel) * nevt          # generator's static (algorithmic) count, FMA = 2
+    executed = float(info.flops_executed_per_event_goodhel) * nevt   # including diagram-group recomputation
+    achieved = flops_call * steps / t_sigma
+    fp64 = prec == mg.FP64
+    peak_meas = peaks["dfma" if fp64 else "ffma"]
+    peak_nom = NOMINAL_FP64 if fp64 else NOMINAL_FP32
+    peak = max(peak_meas, peak_nom)                                  # the larger of measured and nominal
+    traffic = dram_traffic(name, args.precision)
+    mom_bytes = host_mom.numel() * 8
+    out = {
+        "value": nevt * world * steps / t_total, "ms_per_step": t_total / steps * 1e3, "steps": steps, "warmup": warm,
+        "config": config_dict(name, cfg, world, args.precision),
+        "sigma_only": {"value": nevt * world * steps / t_sigma, "unit": UNIT, "ms": t_sigma / steps * 1e3},
+        "rambo": {"ms": t_rambo / steps * 1e3, "bound": "hbm", "bytes_written": mom_bytes,
+                  "achieved_gbs": mom_bytes * steps / t_rambo / 1e9},
+        "e2e": {"value": nevt * world / t_e2e, "unit": UNIT, "h2d_bytes_per_step": mom_bytes,
+                "d2h_bytes_per_step": host_me.numel() * host_me.element_size(), "ms": t_e2e * 1e3,
+                "api": "mg_sigma_host (pinned host momenta in, |M|^2 out)"},
+        "gpu_launches": launches_per_step * steps,
+        "roofline": {"bound": "alu", "achieved": achieved / 1e12, "peak": peak / 1e12, "unit": "TFLOP/s",
+                     "frac": achieved / peak,
+                     "peak_measured_fma_loop": peak_meas / 1e12, "peak_nominal": peak_nom / 1e12,
+                     "peak_dmma_measured": peaks["dmma"] / 1e12,
+                     "peak_source": "max(nominal 148 SM x %d lanes x 2 x 1.965 GHz, %s loop measured in this run with "
+                                    "libmg5b200_peak.so); MEASURED_PEAKS.json has no FP64/FP32 ALU entry"
+                                    % (64 if fp64 else 128, "DFMA" if fp64 else "FFMA"),
+                     "traffic": None if traffic is None or args.nevt else traffic[0],
+                     "traffic_unit": "bytes per mg_sigma call (dram read + write, all its kernels)",
+                     "traffic_source": None if traffic is None or args.nevt else traffic[1],
+                     "algorithmic_bytes": nevt * (32 * info.npar + me.element_size()),
+                     "kernel": "mg_sigma: all kernels of one call, timed together with CUDA events (%d launches)"
+                               % int(info.launches_last_sigma),
+                     "flops_per_event": int(info.flops_per_event_goodhel), "ngoodhel": int(info.ngoodhel),
+                     "nhel_evaluated": int(info.nhel_evaluated),
+                     "executed_tflops": executed * steps / t_sigma / 1e12,
+                     "executed_frac": executed * steps / t_sigma / peak,
+                     "executed_flops_per_event": int(info.flops_executed_per_event_goodhel),
+                     "workspace_bytes": int(info.workspace_bytes)},
+        "clocks": clocks,
+    }
+    proc.close()
+    del mom, me, flush
+    torch.cuda.empty_cache()
+    return out
+
+
 def main():
     args = parse()
     name = args.workload
@@ -172,115 +311,34 @@ def main():
     if world > 1:
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-
-    prec = mg.FP64 if args.precision == "fp64" else mg.FP32
-    proc = mg.Process(cfg["proc"], precision=prec, device=local)
-    nevt = cfg["nevt"]
-    first, _ = mg.shard(nevt, rank, world)
-    st = torch.cuda.current_stream()
-    mom = proc.alloc_momenta(nevt)
-    me = torch.empty(nevt, dtype=torch.float64 if prec == mg.FP64 else torch.float32, device=mom.device)
-    flush = torch.empty(256 << 20, dtype=torch.uint8, device=mom.device)
-
-    # set-up outside the timed region: helicity probe (K8), FMA peak measurement
-    proc.rambo(cfg["seed"], cfg["sqrt_s"], nevt, first_event=first, out=mom)
-    proc.helicity_probe(mom, min(nevt, 4096))
-    info = proc.info
-    peak64 = mg.fma_peak(local, prec)
-
-    def step(ev=None):
-        if ev:
-            ev[0].record(st)
-        proc.rambo(cfg["seed"], cfg["sqrt_s"], nevt, first_event=first, out=mom, stream=st)
-        if ev:
-            ev[1].record(st)
-        proc.sigma(mom, nevt, out=me, stream=st)
-        if ev:
-            ev[2].record(st)
-
-    for _ in range(max(args.warmup, 3)):
-        step()
-    torch.cuda.synchronize()
-    sampler = ClockSampler(local)
-    if rank == 0:
-        sampler.start()
-    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
-    if dist:
-        dist.barrier()
-    torch.cuda.synchronize()
-    for k in range(args.steps):
-        flush.fill_(k & 0xFF)             # L2 flush between timed steps (not timed)
-        step(evs[k])
-    torch.cuda.synchronize()
-    if dist:
-        dist.barrier()
-    t_rambo = sum(e[0].elapsed_time(e[1]) for e in evs) * 1e-3
-    t_sigma = sum(e[1].elapsed_time(e[2]) for e in evs) * 1e-3
-    t_total = t_rambo + t_sigma
-
-    # e2e: host buffers through the C ABI (mg_sigma_host): H2D of the momenta + D2H of |M|^2 in the timed region
-    host_mom = torch.empty(mom.numel(), dtype=torch.float64).pin_memory()
-    host_mom.copy_(mom)
-    host_me = torch.empty(nevt, dtype=me.dtype).pin_memory()
-    ne2e = max(3, min(args.steps, 5))
-    proc.sigma_host(host_mom, nevt, out_host=host_me)
-    torch.cuda.synchronize()
-    if dist:
-        dist.barrier()
-    t0 = time.perf_counter()
-    for _ in range(ne2e):
-        proc.sigma_host(host_mom, nevt, out_host=host_me)      # synchronises internally
-    t_e2e = (time.perf_counter() - t0) / ne2e
-    clocks = sampler.stop() if rank == 0 else None
-    assert torch.equal(host_me.cuda(), me), "host and device entry points disagree"
-
-    if dist:
-        t = torch.tensor([t_total, t_sigma, t_rambo, t_e2e], dtype=torch.float64, device=mom.device)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        t_total, t_sigma, t_rambo, t_e2e = [float(x) for x in t]
+    peaks = measured_peaks(local)
+    res = measure(mg, torch, dist, name, cfg, args, args.steps, rank, world, local, peaks, True)
+    also = {}
+    if name == "ggttgg" and not args.nevt and not args.single:
+        # BASELINE.json's metric is quoted on two processes: the second one, g g > t t~ g g g (configs[4]), is timed
+        # in the same invocation and reported under "also"
+        also["ggttggg"] = measure(mg, torch, dist, "ggttggg", dict(workloads.CONFIGS["ggttggg"]), args,
+                                  max(3, min(args.steps, 5)), rank, world, local, peaks, True)
     if rank != 0:
         if dist:
             dist.destroy_process_group()
         return 0
-
-    info = proc.info
-    launches_per_step = int(info.launches_last_sigma) + 1            # the sigma kernels + the RAMBO kernel
-    flops_launch = float(info.flops_per_event_goodhel) * nevt        # generator's static (algorithmic) count, FMA = 2
-    executed = float(info.flops_executed_per_event_goodhel) * nevt   # including diagram-group recomputation
-    achieved = flops_launch * args.steps / t_sigma
-    traffic = DRAM_TRAFFIC.get((name, args.precision))
-    value = nevt * world * args.steps / t_total
-    line = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
-        "ms_per_step": t_total / args.steps * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "f64" if prec == mg.FP64 else "f32", "data": "synthetic", "config": config_dict(name, cfg, world, args.precision),
-        "sigma_only": {"value": nevt * world * args.steps / t_sigma, "unit": UNIT, "ms": t_sigma / args.steps * 1e3},
-        "rambo_ms": t_rambo / args.steps * 1e3,
-        "e2e": {"value": nevt * world / t_e2e, "unit": UNIT, "h2d_bytes_per_step": host_mom.numel() * 8,
-                "d2h_bytes_per_step": host_me.numel() * host_me.element_size(), "ms": t_e2e * 1e3,
-                "api": "mg_sigma_host (pinned host momenta in, |M|^2 out)"},
-        "gpu_launches": launches_per_step * args.steps,
-        "roofline": {"bound": "alu", "achieved": achieved / 1e12, "peak": peak64 / 1e12, "unit": "TFLOP/s",
-                     "frac": achieved / peak64,
-                     "traffic": None if traffic is None or args.nevt else traffic[0],
-                     "traffic_unit": "bytes per mg_sigma call (dram read + write, all its kernels)",
-                     "traffic_source": None if traffic is None or args.nevt else traffic[1],
-                     "algorithmic_bytes": nevt * (32 * info.npar + me.element_size()),
-                     "kernel": "mg_sigma: all amplitude (diagram-group), gather, colour and helicity-sum kernels of one "
-                               "call, timed together with CUDA events (%d launches)" % int(info.launches_last_sigma),
-                     "flops_per_event": int(info.flops_per_event_goodhel), "ngoodhel": int(info.ngoodhel),
-                     "executed_tflops": executed * args.steps / t_sigma / 1e12,
-                     "executed_frac": executed * args.steps / t_sigma / peak64,
-                     "executed_flops_per_event": int(info.flops_executed_per_event_goodhel),
-                     "peak_source": "mg_fma_peak measured in this run (%s FMA loop on all SMs); MEASURED_PEAKS.json has no "
-                                    "FP64 entry" % ("DFMA" if prec == mg.FP64 else "FFMA")},
-        "clocks": clocks,
-    }
+    line = {"metric": METRIC, "value": res.pop("value"), "unit": UNIT, "n_gpus": world, "steps": res.pop("steps"),
+            "warmup": res.pop("warmup"), "ms_per_step": res.pop("ms_per_step"), "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64" if args.precision == "fp64" else "f32", "data": "synthetic"}
+    line.update(res)
+    if also:
+        line["also"] = also
     if not args.no_cpu_baseline:
         ns = ORACLE_SAMPLE[name]
         v, dt, cores = oracle_time(name, cfg, ns)
         line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "seconds": dt,
                                 "sample": "first %d events of the workload's seeded RAMBO batch, |M|^2 only" % ns}
+        for nm in also:
+            ns2 = ORACLE_SAMPLE[nm]
+            v2, dt2, cores2 = oracle_time(nm, workloads.CONFIGS[nm], ns2)
+            also[nm]["cpu_baseline"] = {"value": v2, "unit": UNIT, "cores": cores2, "kind": "oracle", "seconds": dt2,
+                                        "sample": "first %d events of the workload's seeded RAMBO batch, |M|^2 only" % ns2}
     print(json.dumps(line), flush=True)
     if dist:
         dist.destroy_process_group()

@@ -66,15 +66,19 @@ typedef struct {          /* caller-owned, copied by mg_process_create          
 
 typedef struct {
   int32_t npar, nfinal, ndiagrams, nhel, ngoodhel, ncolor, denominator, nepp;
-  int64_t flops_per_event_allhel;  /* generator's static FLOP count (FMA = 2), all helicities: the method's */
-                                   /* own (algorithmic) count, every current computed once per helicity    */
-  int64_t flops_per_event_goodhel; /* same for the current good-helicity list                              */
-  double masses[8];                /* per particle, process order                                   */
-  int32_t nkernels_per_tile;       /* kernel launches mg_sigma makes per event tile (1 = fused kernel)      */
-  int32_t launches_last_sigma;     /* kernels launched by the last mg_sigma call on this handle             */
-  int64_t workspace_bytes;         /* library-owned JAMP workspace currently allocated (split kernels only) */
-  int64_t flops_executed_per_event_goodhel; /* FLOPs the kernels execute, including the currents that      */
-                                   /* diagram-group kernels recompute (>= flops_per_event_goodhel)          */
+  int64_t flops_per_event_allhel;  /* generator's static FLOP count (FMA = 2) with all 2^npar helicities evaluated: */
+                                   /* the method's own (algorithmic) count — every current computed once per        */
+                                   /* helicity, the tabled low-multiplicity currents once per event                 */
+  int64_t flops_per_event_goodhel; /* same for the helicities evaluated now (nhel_evaluated)                        */
+  double masses[8];                /* per particle, process order                                                   */
+  int32_t nkernels_per_tile;       /* kernel launches mg_sigma makes per event tile (1 = fused kernel)              */
+  int32_t launches_last_sigma;     /* kernels launched by the last mg_sigma call on this handle                     */
+  int64_t workspace_bytes;         /* workspace currently attached (library-owned or caller-provided)               */
+  int64_t flops_executed_per_event_goodhel; /* FLOPs the kernels execute, including the currents that diagram      */
+                                   /* groups recompute (>= flops_per_event_goodhel)                                 */
+  int32_t nhel_evaluated;          /* helicities evaluated per event: a good helicity whose helicity-flipped mirror */
+                                   /* has the same |M_h|^2 on the probe batch is evaluated once and counted twice   */
+  int32_t reserved;
 } mg_info_t;
 
 /* Fills *params with the defaults of BASELINE.json's configs (fp64, helicity filter, device 0). */
@@ -103,17 +107,37 @@ int mg_philox_raw(mg_process_t* p, uint64_t seed, int64_t first_event, int64_t n
 /* K3..K7: |M|^2 for nevt events.  momenta_dev: layout above; me_out_dev: nevt doubles (MG_FP64) or floats
  * (MG_FP32).  Asynchronous on `stream`, except that in MG_HEL_FILTER mode the first call runs the
  * helicity probe (K8) on the first min(nevt, 4096) events and synchronises the stream once, and that the
- * processes with >= 24 colour flows keep partial JAMPs in a library-owned workspace (at most MG5B200_WS_GB
- * GiB, default min(64, 40 % of the free device memory); larger batches are processed in event tiles and helicity chunks) which is (re)allocated, synchronously, by
- * the first call that needs a bigger one. */
+ * processes with >= 24 colour flows use a workspace (per-event invariants of one event tile + the L2-resident JAMP
+ * scratch of the resident CTAs): library-owned by default — at most 1 GiB, larger batches are processed in event
+ * tiles; (re)allocated, synchronously, by the first call that needs a bigger one — or caller-provided
+ * (mg_set_workspace).  One handle serves one stream at a time: the workspace and the helicity lists belong to the
+ * handle, so calls on the same handle must be ordered by the caller (distinct handles are independent). */
 int mg_sigma(mg_process_t* p, const void* momenta_dev, int64_t nevt, void* me_out_dev, void* stream);
+
+/* Caller-provided workspace: `workspace_dev` (256-byte aligned device memory, `bytes` long) replaces
+ * the library-owned one; the library never frees it; NULL returns to the library-owned workspace.
+ * mg_workspace_bytes(p, nevt) is the size with which a batch of nevt events runs as one tile (0 for the processes
+ * that need none); anything >= mg_workspace_bytes(p, 32) works (smaller tiles).  MG_ERR_BAD_PARAM if too small. */
+int mg_set_workspace(mg_process_t* p, void* workspace_dev, size_t bytes);
+size_t mg_workspace_bytes(const mg_process_t* p, int64_t nevt);
+
+/* Batch-unweighting primitive (PAPER.md:99-:103, Table 2 :119-:127: "weights from Jacobian terms and PDFs are
+ * transferred to the GPU, and multiplied with the matrix elements that are already in GPU memory ... The maximum of
+ * these weights is computed in parallel"): me_dev[i] <- weights_dev[i] * me_dev[i] in place (me_dev: the output of
+ * mg_sigma, element type of the handle's precision; weights_dev: nevt doubles) and
+ *     out_dev[0] = max_i, out_dev[1] = sum_i, out_dev[2] = sum_i of squares        of the products (doubles).
+ * Fixed reduction tree: results are bit-reproducible.  nevt = 0 gives (-inf, 0, 0).  Asynchronous on `stream`. */
+int mg_weight_max(mg_process_t* p, void* me_dev, const double* weights_dev, int64_t nevt, double* out_dev, void* stream);
 
 /* Same from HOST buffers (momenta_host: layout above, me_out_host: nevt elements; pinned memory recommended): copies
  * in, runs, copies out and synchronises.  The device staging buffers belong to the handle, grow on demand and are
  * freed by mg_process_destroy.  This is the end-to-end entry point bench.py times as `e2e`. */
 int mg_sigma_host(mg_process_t* p, const void* momenta_host, int64_t nevt, void* me_out_host, void* stream);
 
-/* K8: explicit helicity probe on nprobe events; sets the good-helicity list (synchronises). */
+/* K8: explicit helicity probe on nprobe events; sets the good-helicity list (h is good iff its share of the summed
+ * |M|^2 of the probe batch exceeds 1e-14, 1e-6 in fp32) and finds the helicities whose helicity-flipped mirror has
+ * the same |M_h|^2 on every probe event (parity invariance of QCD; not e+ e- -> mu+ mu-): those are evaluated once
+ * and counted twice.  The statistics are reduced on the device; synchronises.  A no-op on MG_HEL_ALL handles. */
 int mg_helicity_probe(mg_process_t* p, const void* momenta_dev, int64_t nprobe, void* stream);
 /* Per-helicity |M_h|^2 (already divided by the denominator), all 2^npar helicities:
  * perhel_out_dev[h * nevt + ievt].  Diagnostic / test entry point. */
@@ -124,16 +148,6 @@ int mg_good_helicities(const mg_process_t* p, int32_t* out, int32_t capacity, in
 
 int mg_process_info(const mg_process_t* p, mg_info_t* out);
 size_t mg_momenta_bytes(const mg_process_t* p, int64_t nevt);
-
-/* Measures the sustained FP64 (prec = MG_FP64) or FP32 FMA rate of the device with a dependent-chain-free
- * FMA loop on every SM: the denominator of the "% of peak" figure.  Returns FLOP/s in
- * *flops_per_s; synchronises. */
-int mg_fma_peak(int device, int prec, double* flops_per_s);
-
-/* Same for the FP64 tensor cores: sustained rate of mma.sync.m8n8k4.f64 (DMMA.8x8x4, the native FP64 MMA shape of
- * sm_100a), 8 independent accumulators per warp, 64 warps per SM.  Decides whether the colour contraction (K6) belongs
- * on the tensor cores.  Returns FLOP/s in *flops_per_s; synchronises. */
-int mg_dmma_peak(int device, double* flops_per_s);
 
 const char* mg_status_string(int status);
 const char* mg_last_error(void); /* thread-local detail of the last MG_ERR_CUDA */

@@ -13,14 +13,14 @@ import ctypes as C
 import os
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.environ.get("MG5B200_LIB") or os.path.join(_HERE, "libmg5b200.so")   # override: kernel experiments
+LIB_PATH = os.path.join(_HERE, "libmg5b200.so")
 NEPP = 32
 FP64, FP32 = 0, 1
 HEL_FILTER, HEL_ALL = 0, 1
 
 SYMBOLS = ["mg_params_default", "mg_process_create", "mg_process_destroy", "mg_rambo", "mg_rambo_ex", "mg_philox_raw", "mg_sigma",
            "mg_sigma_host", "mg_helicity_probe", "mg_sigma_per_helicity", "mg_good_helicities", "mg_process_info",
-           "mg_momenta_bytes", "mg_fma_peak", "mg_dmma_peak", "mg_status_string", "mg_last_error"]
+           "mg_momenta_bytes", "mg_set_workspace", "mg_workspace_bytes", "mg_weight_max", "mg_status_string", "mg_last_error"]
 
 
 class MgParams(C.Structure):
@@ -35,7 +35,8 @@ class MgInfo(C.Structure):
                 ("ngoodhel", C.c_int32), ("ncolor", C.c_int32), ("denominator", C.c_int32), ("nepp", C.c_int32),
                 ("flops_per_event_allhel", C.c_int64), ("flops_per_event_goodhel", C.c_int64),
                 ("masses", C.c_double * 8), ("nkernels_per_tile", C.c_int32), ("launches_last_sigma", C.c_int32),
-                ("workspace_bytes", C.c_int64), ("flops_executed_per_event_goodhel", C.c_int64)]
+                ("workspace_bytes", C.c_int64), ("flops_executed_per_event_goodhel", C.c_int64),
+                ("nhel_evaluated", C.c_int32), ("reserved", C.c_int32)]
 
 
 class MgError(RuntimeError):
@@ -69,8 +70,10 @@ def lib():
         L.mg_process_info.argtypes = [vp, C.POINTER(MgInfo)]
         L.mg_momenta_bytes.argtypes = [vp, i64]
         L.mg_momenta_bytes.restype = C.c_size_t
-        L.mg_fma_peak.argtypes = [C.c_int, C.c_int, C.POINTER(C.c_double)]
-        L.mg_dmma_peak.argtypes = [C.c_int, C.POINTER(C.c_double)]
+        L.mg_set_workspace.argtypes = [vp, vp, C.c_size_t]
+        L.mg_workspace_bytes.argtypes = [vp, i64]
+        L.mg_workspace_bytes.restype = C.c_size_t
+        L.mg_weight_max.argtypes = [vp, vp, vp, i64, vp, vp]
         L.mg_status_string.argtypes = [C.c_int]
         L.mg_status_string.restype = C.c_char_p
         L.mg_last_error.restype = C.c_char_p
@@ -94,20 +97,6 @@ def default_params(precision=FP64, helicity_mode=HEL_FILTER, device=0, **kw):
     for k, v in kw.items():
         setattr(p, k, v)
     return p
-
-
-def fma_peak(device=0, precision=FP64):
-    """Measured FMA rate (FLOP/s) of the device: the denominator of '% of FP64 peak'."""
-    out = C.c_double()
-    _check(lib().mg_fma_peak(device, precision, C.byref(out)))
-    return out.value
-
-
-def dmma_peak(device=0):
-    """Measured FP64 tensor-core (DMMA m8n8k4) rate of the device in FLOP/s."""
-    out = C.c_double()
-    _check(lib().mg_dmma_peak(device, C.byref(out)))
-    return out.value
 
 
 def _stream_ptr(stream):
@@ -202,6 +191,27 @@ class Process:
     def helicity_probe(self, momenta, nprobe, stream=None):
         _check(lib().mg_helicity_probe(self._h, C.c_void_p(momenta.data_ptr()), nprobe, _stream_ptr(stream)))
         return self.good_helicities()
+
+    def set_workspace(self, buf):
+        """mg_set_workspace: `buf` = a CUDA tensor the caller keeps alive (None: back to the library-owned workspace)."""
+        if buf is None:
+            _check(lib().mg_set_workspace(self._h, None, 0))
+        else:
+            _check(lib().mg_set_workspace(self._h, C.c_void_p(buf.data_ptr()), buf.numel() * buf.element_size()))
+        self._ws_keepalive = buf
+
+    def workspace_bytes(self, nevt):
+        return int(lib().mg_workspace_bytes(self._h, nevt))
+
+    def weight_max(self, me, weights, nevt=None, out=None, stream=None):
+        """mg_weight_max: me <- weights * me in place; returns the device tensor (max, sum, sum of squares)."""
+        import torch
+        nevt = me.numel() if nevt is None else nevt
+        assert me.is_cuda and weights.is_cuda and weights.dtype == torch.float64 and me.dtype == self._out_dtype()
+        res = out if out is not None else torch.empty(3, dtype=torch.float64, device=me.device)
+        _check(lib().mg_weight_max(self._h, C.c_void_p(me.data_ptr()), C.c_void_p(weights.data_ptr()), nevt,
+                                   C.c_void_p(res.data_ptr()), _stream_ptr(stream)))
+        return res
 
     def good_helicities(self):
         n = C.c_int32()

@@ -2,11 +2,15 @@
 
     python -m paper_2312_02898_b200.build [--force]
 
-Generated sources go to csrc/generated/ (git-ignored: they are a pure function of gen/); objects to
-csrc/build/; the shared library next to this file.  nvcc cross-compiles without a GPU.
+Generated sources go to csrc/generated/ (git-ignored: they are a pure function of gen/); objects and the per-unit
+`ptxas -v` logs to csrc/build/; the shared library next to this file.  Everything is compiled as relocatable device
+code (-rdc=true): the diagram-group bodies of the event-CTA kernels are separate translation units linked into one
+kernel.  nvcc cross-compiles without a GPU.  `python -m paper_2312_02898_b200.build --resources` prints the
+registers / spill / stack table of the compiled units (from the ptxas logs).
 """
 import hashlib
 import os
+import re
 import subprocess
 import sys
 from concurrent.futures import ThreadPoolExecutor
@@ -16,47 +20,25 @@ CSRC = os.path.join(HERE, "csrc")
 GEN = os.path.join(CSRC, "generated")
 OBJ = os.path.join(CSRC, "build")
 LIB = os.path.join(HERE, "libmg5b200.so")
+PEAK_LIB = os.path.join(HERE, "libmg5b200_peak.so")     # measurement helper for bench.py (csrc/peak), not the product
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
-FLAGS = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", "-I", CSRC] + os.environ.get("MG_NVCC_EXTRA", "").split()
+FLAGS = ["-O3", "-std=c++17", "-lineinfo", "-rdc=true", "-Xcompiler", "-fPIC", "-I", CSRC]
+HAND = ("mg_api.cu", "mg_rambo.cu", "mg_reduce.cu")
 
 
-def generate():
-    """Runs the process generator; returns (list of generated .cu paths, list of info dicts)."""
+def generate(overrides=None):
+    """Runs the process generator; returns (list of generated .cu paths, list of info dicts).  `overrides`
+    (tuning runs only): {n_gluons: dict of emit_coop keyword overrides}."""
     import json
     from .gen.emit import emit_eemumu, emit_ggttng
     os.makedirs(GEN, exist_ok=True)
     infos, paths = [], []
-    ns_gluons = [int(x) for x in os.environ.get("MG_NGLUONS", "2,3,4,5").split(",") if x]
-    shapes = dict(kv.split("=") for kv in os.environ.get("MG_SHAPES", "").split(",") if kv)   # e.g. "4=fused"
-    maxterms = dict(kv.split("=") for kv in os.environ.get("MG_MAXTERMS", "").split(",") if kv)   # e.g. "4=40"
-    block = dict(kv.split("=") for kv in os.environ.get("MG_BLOCK", "").split(",") if kv)
     jobs = [emit_eemumu()]
-    for n in ns_gluons:
+    for n in (2, 3, 4, 5):
         kw = dict(fp32=(n < 5))
-        if os.environ.get("MG_ACCMAX"):
-            kw["acc_max"] = int(os.environ["MG_ACCMAX"])
-        if str(n) in block:
-            kw["block"] = int(block[str(n)])
-        if str(n) in maxterms:
-            kw["max_terms"] = int(maxterms[str(n)])
-        if os.environ.get("MG_PREFETCH"):
-            kw["prefetch"] = int(os.environ["MG_PREFETCH"])
-        if os.environ.get("MG_REDUCE"):
-            kw["reduce_mode"] = os.environ["MG_REDUCE"]
-        if os.environ.get("MG_STAGEKB"):
-            kw["stage_kb"] = int(os.environ["MG_STAGEKB"])
-        if os.environ.get("MG_NOINLINE"):
-            kw["noinline"] = os.environ["MG_NOINLINE"] == "1"
-        if os.environ.get("MG_FLAT") and n >= 5:
-            kw["flat_phase"] = int(os.environ["MG_FLAT"])
-        if os.environ.get("MG_LIVEMAX"):
-            kw["live_max"] = int(os.environ["MG_LIVEMAX"])
-        if os.environ.get("MG_SYNC"):
-            kw["sync_every"] = int(os.environ["MG_SYNC"])
-        if os.environ.get("MG_MINBLOCKS"):
-            kw["minblocks"] = int(os.environ["MG_MINBLOCKS"])
-        jobs.append(emit_ggttng(n, shape=shapes.get(str(n)), **kw))
+        kw.update((overrides or {}).get(n, {}))
+        jobs.append(emit_ggttng(n, **kw))
     keep = set()
     for files, info in jobs:
         for fname, src in files:
@@ -119,20 +101,49 @@ def _compile(path, force, log):
     return obj
 
 
-def build(force=False, log=True):
-    gen_paths, infos = generate()
-    hand = [os.path.join(CSRC, f) for f in ("mg_api.cu", "mg_rambo.cu", "mg_peak.cu")]
+def build(force=False, log=True, overrides=None):
+    gen_paths, infos = generate(overrides)
+    hand = [os.path.join(CSRC, f) for f in HAND]
     srcs = sorted(gen_paths, key=lambda p: -os.path.getsize(p)) + hand    # largest first
     with ThreadPoolExecutor(max_workers=min(8, os.cpu_count() or 1)) as ex:
         objs = list(ex.map(lambda p: _compile(p, force, log), srcs))
+    for f in os.listdir(OBJ):            # objects of units that no longer exist
+        if f.endswith(".o") and os.path.join(OBJ, f) not in objs:
+            for ext in ("", ".stamp"):
+                if os.path.exists(os.path.join(OBJ, f + ext)):
+                    os.remove(os.path.join(OBJ, f + ext))
     newest = max(os.path.getmtime(o) for o in objs)
     if force or not os.path.exists(LIB) or os.path.getmtime(LIB) < newest:
-        cmd = [NVCC] + ARCH + ["-shared", "-o", LIB] + objs + ["-lcudart"]
+        cmd = [NVCC] + ARCH + ["-rdc=true", "-shared", "-o", LIB] + objs + ["-lcudart"]
         subprocess.check_call(cmd)
         if log:
             print("linked", LIB, flush=True)
+    peak_src = os.path.join(CSRC, "peak", "mg_peak.cu")
+    if force or not os.path.exists(PEAK_LIB) or os.path.getmtime(PEAK_LIB) < os.path.getmtime(peak_src):
+        subprocess.check_call([NVCC] + ARCH + ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", "-shared", "-o", PEAK_LIB,
+                                               peak_src, "-lcudart"])
     return LIB
 
 
+def resources():
+    """Registers / stack / spill per compiled entry or device function, parsed from the ptxas -v logs."""
+    rows = []
+    for f in sorted(os.listdir(OBJ)):
+        if not f.endswith(".ptxas.log"):
+            continue
+        txt = open(os.path.join(OBJ, f)).read()
+        for m in re.finditer(r"Compiling entry function '(\S+)'.*?\n(?:ptxas info\s*:.*\n)*?ptxas info\s*: Function properties for \S+\n"
+                             r"\s*(\d+) bytes stack frame, (\d+) bytes spill stores, (\d+) bytes spill loads\n"
+                             r"ptxas info\s*: Used (\d+) registers", txt):
+            rows.append((f[:-10], m.group(1), int(m.group(5)), int(m.group(2)), int(m.group(3)), int(m.group(4))))
+        for m in re.finditer(r"Function properties for (\S+)\n\s*(\d+) bytes stack frame, (\d+) bytes spill stores, (\d+) bytes spill loads", txt):
+            rows.append((f[:-10], m.group(1), None, int(m.group(2)), int(m.group(3)), int(m.group(4))))
+    return rows
+
+
 if __name__ == "__main__":
-    build(force="--force" in sys.argv)
+    if "--resources" in sys.argv:
+        for r in resources():
+            print("%-22s %-60s regs=%s stack=%d spill_st=%d spill_ld=%d" % r)
+    else:
+        build(force="--force" in sys.argv)

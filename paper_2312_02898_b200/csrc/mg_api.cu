@@ -1,5 +1,5 @@
 // mg_api.cu — the C ABI of include/mg5b200.h: argument checking, handle management, helicity filter (K8),
-// and dispatch to the generated per-process launchers.  No arithmetic of the method lives here.
+// workspace, and dispatch to the generated per-process launchers.  No arithmetic of the method lives here.
 #include <math.h>
 #include <stdio.h>
 #include <stdlib.h>
@@ -20,47 +20,68 @@ static int cuda_fail(cudaError_t e, const char* where) {
   snprintf(g_err, sizeof g_err, "%s: %s", where, cudaGetErrorString(e));
   return MG_ERR_CUDA;
 }
+static int fail(int status, const char* what) {
+  snprintf(g_err, sizeof g_err, "%s", what);
+  return status;
+}
 #define MG_CUDA(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cuda_fail(e_, #call); } while (0)
 
 struct mg_process {
-  const mg_procdesc_t* desc;
+  const mg_procdesc_t* desc = nullptr;
   mg_params_t par;
   double pvec[MG_NPAR_VEC];
   double masses[8];
-  int nfinal;
-  int* hel_dev;            // good-helicity list on the device (nhel ints)
-  int* hel_all_dev;        // 0..nhel-1
-  std::vector<int> good;
-  bool probed;
-  long long launches;      // kernels launched by the last mg_sigma / mg_sigma_per_helicity call
-  void* io_mom; size_t io_mom_bytes;   // device staging of mg_sigma_host (grow-only, library-owned)
-  void* io_out; size_t io_out_bytes;
-  void* ws;                // workspace of the split kernel shape (JAMPs + per-helicity values), library-owned
-  size_t ws_bytes;
+  int nfinal = 0, nsm = 0;
+  // helicity state (K8).  good: helicities that contribute; run: the ones evaluated, with weights (2 = stands for its
+  // helicity-flipped mirror as well, which is then not evaluated)
+  std::vector<int> good, run;
+  std::vector<double> run_w;
+  bool probed = false;
+  int* hel_dev = nullptr;        // fused shape: run list / all helicities
+  int* hel_all_dev = nullptr;
+  double* helw_dev = nullptr;    // fused shape: weights of the run list / ones
+  double* ones_dev = nullptr;
+  void* lanew_dev = nullptr;     // event-CTA shape: lane weights [2][nlane] (element type of the precision) / ones
+  void* lanew_all_dev = nullptr;
+  int ntb = 2, tb_first = 0;     // event-CTA shape: top-quark helicities run
+  double* stats_dev = nullptr;   // probe statistics [2][nhel]; first 3 doubles double as mg_weight_max's default output
+  double* wpart_dev = nullptr;   // mg_weight_max stage-1 partials
+  long long launches = 0;        // kernels launched by the last mg_sigma / mg_sigma_per_helicity call
+  void* io_mom = nullptr; size_t io_mom_bytes = 0;   // device staging of mg_sigma_host (grow-only, library-owned)
+  void* io_out = nullptr; size_t io_out_bytes = 0;
+  void* ws = nullptr; size_t ws_bytes = 0; bool ws_user = false;   // event-CTA shape: JAMP scratch + per-event invariants
 };
 
-// Workspace for the split kernel shape: jamp[nhel_run][ncol][2][tile] + meh[nhel_run][tile]; the generated launcher
-// tiles the batch so that it fits.  Capped at MG5B200_WS_GB GiB (default: min(64, 40 % of free memory)).  Grows on demand (synchronous
-// cudaFree/cudaMalloc on the first call that needs more), never shrinks.
-static int ensure_ws(mg_process* p, int64_t nevt, int nhel_run) {
-  const int ip = p->par.precision == MG_FP64 ? 0 : 1;
-  const size_t per_eh = (size_t)p->desc->ws_bytes_per_event_hel[ip], per_e = (size_t)p->desc->ws_bytes_per_event[ip];
-  if (per_eh == 0) return MG_OK;
-  // default cap: 64 GiB or 40 % of the free device memory, whichever is smaller (B200: 180 GB)
-  double cap_gb = 64.0;
-  size_t free_b = 0, total_b = 0;
-  if (cudaMemGetInfo(&free_b, &total_b) == cudaSuccess) {
-    const double f = 0.4 * (double)(free_b + p->ws_bytes) / 1073741824.0;
-    if (f < cap_gb) cap_gb = f;
-  }
-  if (const char* e = getenv("MG5B200_WS_GB")) { const double v = atof(e); if (v > 0) cap_gb = v; }
-  const size_t cap = (size_t)(cap_gb * 1073741824.0);
-  size_t E = (size_t)((nevt + 31) / 32 * 32);
-  if (E > ((size_t)1 << 20)) E = (size_t)1 << 20;             // the launcher's largest event tile
-  size_t need = E * (per_e + (size_t)nhel_run * per_eh);      // whole batch, whole helicity list resident
-  if (need > cap) need = cap;
-  const size_t floor_bytes = (E < 1024 ? E : 1024) * (per_e + 4 * per_eh);
-  if (need < floor_bytes) need = floor_bytes;
+static size_t esize(const mg_process_t* p) { return p->par.precision == MG_FP64 ? 8 : 4; }
+
+static void free_all(mg_process* p) {
+  cudaFree(p->hel_dev); cudaFree(p->hel_all_dev); cudaFree(p->helw_dev); cudaFree(p->ones_dev);
+  cudaFree(p->lanew_dev); cudaFree(p->lanew_all_dev); cudaFree(p->stats_dev); cudaFree(p->wpart_dev);
+  if (p->ws && !p->ws_user) cudaFree(p->ws);
+  if (p->io_mom) cudaFree(p->io_mom);
+  if (p->io_out) cudaFree(p->io_out);
+  cudaGetLastError();
+}
+
+// Workspace of the event-CTA shape: JAMP scratch for every resident CTA (at most 2 per SM) + the per-event invariants
+// of one event tile.  Library-owned by default: sized for the whole batch, capped at MG_WS_DEFAULT_CAP, grown on
+// demand (synchronously), never shrunk; or caller-provided through mg_set_workspace.
+static const size_t MG_WS_DEFAULT_CAP = (size_t)1 << 30;
+static size_t ws_scratch_bytes(const mg_process* p) {
+  return (size_t)2 * p->nsm * (size_t)p->desc->ws_bytes_per_cta[p->par.precision == MG_FP64 ? 0 : 1];
+}
+static size_t ws_need(const mg_process* p, int64_t nevt) {
+  const size_t per_e = (size_t)p->desc->ws_bytes_per_event[p->par.precision == MG_FP64 ? 0 : 1];
+  return ws_scratch_bytes(p) + per_e * (size_t)((nevt + 31) / 32 * 32);
+}
+static int ensure_ws(mg_process* p, int64_t nevt) {
+  if (!p->desc->launch_slots) return MG_OK;
+  const size_t per_e = (size_t)p->desc->ws_bytes_per_event[p->par.precision == MG_FP64 ? 0 : 1];
+  const size_t floor_bytes = ws_scratch_bytes(p) + per_e * 32;
+  if (p->ws_user) return p->ws_bytes >= floor_bytes ? MG_OK : fail(MG_ERR_BAD_PARAM, "caller-provided workspace too small");
+  size_t need = ws_need(p, nevt);
+  if (need > MG_WS_DEFAULT_CAP) need = MG_WS_DEFAULT_CAP;
+  if (need < floor_bytes + per_e * 4096) need = floor_bytes + per_e * 4096;
   if (p->ws_bytes >= need) return MG_OK;
   if (p->ws) { cudaDeviceSynchronize(); cudaFree(p->ws); p->ws = nullptr; p->ws_bytes = 0; }
   MG_CUDA(cudaMalloc(&p->ws, need));
@@ -72,6 +93,53 @@ static std::string squeeze(const char* s) {
   std::string o;
   for (; *s; ++s) if (!isspace((unsigned char)*s)) o.push_back(*s);
   return o;
+}
+
+// lane index of helicity h in the event-CTA shape: the helicity bits of all particles but the top quark (bit tpos)
+static int lane_of(int h, int tpos) { return ((h >> (tpos + 1)) << tpos) | (h & ((1 << tpos) - 1)); }
+
+// uploads the run list / weights of the current helicity state
+static int upload_helicities(mg_process* p) {
+  const mg_procdesc_t* d = p->desc;
+  if (d->launch) {
+    MG_CUDA(cudaMemcpy(p->hel_dev, p->run.data(), sizeof(int) * p->run.size(), cudaMemcpyHostToDevice));
+    MG_CUDA(cudaMemcpy(p->helw_dev, p->run_w.data(), sizeof(double) * p->run_w.size(), cudaMemcpyHostToDevice));
+    return MG_OK;
+  }
+  const int tpos = d->npar - 3, nl = d->nlane;
+  std::vector<double> w(2 * nl, 0.0);
+  bool any[2] = {false, false};
+  for (size_t i = 0; i < p->run.size(); ++i) {
+    const int h = p->run[i], tb = (h >> tpos) & 1;
+    w[tb * nl + lane_of(h, tpos)] = p->run_w[i];
+    any[tb] = true;
+  }
+  p->ntb = (any[0] && any[1]) ? 2 : 1;
+  p->tb_first = any[1] ? 1 : 0;
+  if (p->par.precision == MG_FP64) {
+    MG_CUDA(cudaMemcpy(p->lanew_dev, w.data(), sizeof(double) * w.size(), cudaMemcpyHostToDevice));
+  } else {
+    std::vector<float> wf(w.begin(), w.end());
+    MG_CUDA(cudaMemcpy(p->lanew_dev, wf.data(), sizeof(float) * wf.size(), cudaMemcpyHostToDevice));
+  }
+  return MG_OK;
+}
+
+static int run_sigma(mg_process* p, const void* mom, int64_t nevt, void* me_out, void* perhel, bool all, cudaStream_t st) {
+  const mg_procdesc_t* d = p->desc;
+  long long n;
+  if (d->launch) {
+    n = all ? d->launch(p->par.precision, (const double*)mom, me_out, nevt, p->hel_all_dev, p->ones_dev, d->nhel, perhel, p->pvec, st)
+            : d->launch(p->par.precision, (const double*)mom, me_out, nevt, p->hel_dev, p->helw_dev, (int)p->run.size(), perhel, p->pvec, st);
+  } else {
+    { const int rc = ensure_ws(p, nevt); if (rc != MG_OK) return rc; }
+    n = all ? d->launch_slots(p->par.precision, (const double*)mom, me_out, nevt, p->lanew_all_dev, 2, 0, perhel, p->pvec, p->ws, p->ws_bytes, st)
+            : d->launch_slots(p->par.precision, (const double*)mom, me_out, nevt, p->lanew_dev, p->ntb, p->tb_first, perhel, p->pvec, p->ws, p->ws_bytes, st);
+  }
+  if (n < 0) { cudaGetLastError(); return fail(MG_ERR_CUDA, n == -2 ? "workspace too small for the kernel's JAMP scratch" : "kernel launch set-up failed"); }
+  p->launches = n;
+  MG_CUDA(cudaGetLastError());
+  return MG_OK;
 }
 
 extern "C" {
@@ -92,8 +160,20 @@ int mg_process_create(const char* proc, const mg_params_t* params, mg_process_t*
   if (params->struct_size != sizeof(mg_params_t)) return MG_ERR_BAD_PARAM;
   if (params->helicity_mode != MG_HEL_FILTER && params->helicity_mode != MG_HEL_ALL) return MG_ERR_BAD_PARAM;
   if (!(params->alpha_s > 0) || !(params->alpha_ew_inv > 0) || !(params->mz > 0) || !(params->mt >= 0) ||
-      params->gamma_t != 0.0)
+      !(params->gamma_z >= 0) || params->gamma_t != 0.0)
     return MG_ERR_BAD_PARAM;
+  // derived couplings (DESIGN.md §3 C2, reading A1)
+  const double pi = 3.14159265358979323846;
+  const double aew = 1.0 / params->alpha_ew_inv;
+  double sw2 = params->sw2;
+  if (!(sw2 > 0)) {
+    if (!(params->gf > 0)) return MG_ERR_BAD_PARAM;
+    const double mz2 = params->mz * params->mz;
+    const double rad = mz2 * mz2 / 4 - pi * aew * mz2 / (sqrt(2.0) * params->gf);
+    if (!(rad >= 0)) return MG_ERR_BAD_PARAM;
+    sw2 = 1.0 - (mz2 / 2 + sqrt(rad)) / mz2;
+  }
+  if (!(sw2 > 0 && sw2 < 1)) return MG_ERR_BAD_PARAM;
   const std::string key = squeeze(proc);
   const mg_procdesc_t* d = nullptr;
   for (int i = 0; i < mg_registry_n; ++i) if (squeeze(mg_registry[i]->proc) == key) d = mg_registry[i];
@@ -106,19 +186,10 @@ int mg_process_create(const char* proc, const mg_params_t* params, mg_process_t*
   }
   MG_CUDA(cudaSetDevice(params->device));
   mg_process* p = new mg_process();
-  p->desc = d; p->par = *params; p->probed = false; p->ws = nullptr; p->ws_bytes = 0; p->launches = 0;
-  p->io_mom = p->io_out = nullptr; p->io_mom_bytes = p->io_out_bytes = 0;
+  p->desc = d; p->par = *params;
   p->nfinal = d->npar - 2;
+  if (cudaDeviceGetAttribute(&p->nsm, cudaDevAttrMultiProcessorCount, params->device) != cudaSuccess) p->nsm = 148;
   for (int i = 0; i < 8; ++i) p->masses[i] = (i < d->npar && d->massive[i]) ? params->mt : 0.0;
-  // derived couplings (DESIGN.md §3 C2, reading A1)
-  const double pi = 3.14159265358979323846;
-  const double aew = 1.0 / params->alpha_ew_inv;
-  double sw2 = params->sw2;
-  if (!(sw2 > 0)) {
-    const double mz2 = params->mz * params->mz;
-    const double mw2 = mz2 / 2 + sqrt(mz2 * mz2 / 4 - pi * aew * mz2 / (sqrt(2.0) * params->gf));
-    sw2 = 1.0 - mw2 / mz2;
-  }
   const double e2 = 4 * pi * aew, e = sqrt(e2);
   const double gz = e / (2 * sqrt(sw2 * (1 - sw2))), gv = -0.5 + 2 * sw2, ga = -0.5;
   memset(p->pvec, 0, sizeof p->pvec);
@@ -129,14 +200,30 @@ int mg_process_create(const char* proc, const mg_params_t* params, mg_process_t*
   p->pvec[MG_PAR_GR] = -gz * (gv - ga);
   p->pvec[MG_PAR_MZ2] = params->mz * params->mz;
   p->pvec[MG_PAR_MZGZ] = params->mz * params->gamma_z;
-  std::vector<int> all(d->nhel);
-  for (int h = 0; h < d->nhel; ++h) all[h] = h;
-  p->good = all;
-  cudaError_t e1 = cudaMalloc(&p->hel_dev, sizeof(int) * d->nhel);
-  cudaError_t e2c = e1 == cudaSuccess ? cudaMalloc(&p->hel_all_dev, sizeof(int) * d->nhel) : e1;
-  if (e2c != cudaSuccess) { delete p; return cuda_fail(e2c, "cudaMalloc(helicity list)"); }
-  cudaMemcpy(p->hel_dev, all.data(), sizeof(int) * d->nhel, cudaMemcpyHostToDevice);
-  cudaMemcpy(p->hel_all_dev, all.data(), sizeof(int) * d->nhel, cudaMemcpyHostToDevice);
+  const int nhel = d->nhel;
+  std::vector<int> all(nhel);
+  for (int h = 0; h < nhel; ++h) all[h] = h;
+  p->good = all; p->run = all; p->run_w.assign(nhel, 1.0);
+  const size_t es = esize(p);
+  std::vector<double> ones(nhel > 2 * d->nlane ? nhel : 2 * d->nlane + 1, 1.0);
+  std::vector<float> onesf(ones.begin(), ones.end());
+  cudaError_t ce = cudaMalloc(&p->stats_dev, sizeof(double) * 2 * nhel);
+  if (ce == cudaSuccess) ce = cudaMalloc(&p->wpart_dev, sizeof(double) * 3 * MG_WEIGHT_MAX_BLOCKS);
+  if (d->launch) {
+    if (ce == cudaSuccess) ce = cudaMalloc(&p->hel_dev, sizeof(int) * nhel);
+    if (ce == cudaSuccess) ce = cudaMalloc(&p->hel_all_dev, sizeof(int) * nhel);
+    if (ce == cudaSuccess) ce = cudaMalloc(&p->helw_dev, sizeof(double) * nhel);
+    if (ce == cudaSuccess) ce = cudaMalloc(&p->ones_dev, sizeof(double) * nhel);
+    if (ce == cudaSuccess) ce = cudaMemcpy(p->hel_all_dev, all.data(), sizeof(int) * nhel, cudaMemcpyHostToDevice);
+    if (ce == cudaSuccess) ce = cudaMemcpy(p->ones_dev, ones.data(), sizeof(double) * nhel, cudaMemcpyHostToDevice);
+  } else {
+    if (ce == cudaSuccess) ce = cudaMalloc(&p->lanew_dev, es * 2 * d->nlane);
+    if (ce == cudaSuccess) ce = cudaMalloc(&p->lanew_all_dev, es * 2 * d->nlane);
+    if (ce == cudaSuccess) ce = cudaMemcpy(p->lanew_all_dev, es == 8 ? (const void*)ones.data() : (const void*)onesf.data(),
+                                           es * 2 * d->nlane, cudaMemcpyHostToDevice);
+  }
+  if (ce != cudaSuccess) { free_all(p); delete p; return cuda_fail(ce, "mg_process_create: device set-up"); }
+  { const int rc = upload_helicities(p); if (rc != MG_OK) { free_all(p); delete p; return rc; } }
   if (params->helicity_mode == MG_HEL_ALL) p->probed = true;
   *out = p;
   return MG_OK;
@@ -145,11 +232,7 @@ int mg_process_create(const char* proc, const mg_params_t* params, mg_process_t*
 int mg_process_destroy(mg_process_t* p) {
   if (!p) return MG_ERR_NULL;
   cudaSetDevice(p->par.device);
-  cudaFree(p->hel_dev);
-  cudaFree(p->hel_all_dev);
-  if (p->ws) cudaFree(p->ws);
-  if (p->io_mom) cudaFree(p->io_mom);
-  if (p->io_out) cudaFree(p->io_out);
+  free_all(p);
   delete p;
   return MG_OK;
 }
@@ -158,6 +241,22 @@ size_t mg_momenta_bytes(const mg_process_t* p, int64_t nevt) {
   if (!p || nevt < 0) return 0;
   const int64_t pages = (nevt + MG_NEPP - 1) / MG_NEPP;
   return (size_t)pages * p->desc->npar * MG_NEPP * 4 * sizeof(double);
+}
+
+size_t mg_workspace_bytes(const mg_process_t* p, int64_t nevt) {
+  if (!p || nevt < 0 || !p->desc->launch_slots) return 0;
+  return ws_need(p, nevt);
+}
+
+int mg_set_workspace(mg_process_t* p, void* workspace_dev, size_t bytes) {
+  if (!p) return MG_ERR_NULL;
+  if ((uintptr_t)workspace_dev & 255) return MG_ERR_ALIGN;
+  MG_CUDA(cudaSetDevice(p->par.device));
+  if (p->ws && !p->ws_user) { cudaDeviceSynchronize(); cudaFree(p->ws); }
+  p->ws = workspace_dev; p->ws_bytes = workspace_dev ? bytes : 0; p->ws_user = workspace_dev != nullptr;
+  if (p->ws_user && p->desc->launch_slots && bytes < mg_workspace_bytes(p, 32))
+    return fail(MG_ERR_BAD_PARAM, "workspace smaller than mg_workspace_bytes(p, 32)");
+  return MG_OK;
 }
 
 int mg_rambo_ex(mg_process_t* p, uint64_t seed, double sqrt_s, int64_t first_event, int64_t nevt,
@@ -186,8 +285,6 @@ int mg_philox_raw(mg_process_t* p, uint64_t seed, int64_t first_event, int64_t n
   return MG_OK;
 }
 
-static size_t esize(const mg_process_t* p) { return p->par.precision == MG_FP64 ? 8 : 4; }
-
 int mg_sigma_per_helicity(mg_process_t* p, const void* momenta_dev, int64_t nevt, void* perhel_out_dev, void* stream) {
   if (!p || ((!momenta_dev || !perhel_out_dev) && nevt > 0)) return MG_ERR_NULL;
   if (nevt < 0) return MG_ERR_BAD_NEVT;
@@ -195,13 +292,11 @@ int mg_sigma_per_helicity(mg_process_t* p, const void* momenta_dev, int64_t nevt
   if (nevt == 0) return MG_OK;
   MG_CUDA(cudaSetDevice(p->par.device));
   void* tmp = nullptr;
-  { const int rc = ensure_ws(p, nevt, p->desc->nhel); if (rc != MG_OK) return rc; }
   MG_CUDA(cudaMalloc(&tmp, esize(p) * (size_t)nevt));
-  p->launches = p->desc->launch(p->par.precision, (const double*)momenta_dev, tmp, nevt, p->hel_all_dev, p->desc->nhel,
-                  perhel_out_dev, p->pvec, p->ws, p->ws_bytes, (cudaStream_t)stream);
-  cudaError_t e = cudaGetLastError();
-  if (e == cudaSuccess) e = cudaStreamSynchronize((cudaStream_t)stream);
+  const int rc = run_sigma(p, momenta_dev, nevt, tmp, perhel_out_dev, true, (cudaStream_t)stream);
+  const cudaError_t e = cudaStreamSynchronize((cudaStream_t)stream);
   cudaFree(tmp);
+  if (rc != MG_OK) return rc;
   if (e != cudaSuccess) return cuda_fail(e, "sigma_per_helicity");
   return MG_OK;
 }
@@ -209,31 +304,45 @@ int mg_sigma_per_helicity(mg_process_t* p, const void* momenta_dev, int64_t nevt
 int mg_helicity_probe(mg_process_t* p, const void* momenta_dev, int64_t nprobe, void* stream) {
   if (!p || !momenta_dev) return MG_ERR_NULL;
   if (nprobe <= 0) return MG_ERR_BAD_NEVT;
+  if (p->par.helicity_mode == MG_HEL_ALL) return MG_OK;       // MG_HEL_ALL handles always sum every helicity
   const int nhel = p->desc->nhel;
   void* ph = nullptr;
   MG_CUDA(cudaSetDevice(p->par.device));
   MG_CUDA(cudaMalloc(&ph, esize(p) * (size_t)nprobe * nhel));
   int rc = mg_sigma_per_helicity(p, momenta_dev, nprobe, ph, stream);
-  if (rc != MG_OK) { cudaFree(ph); return rc; }
-  std::vector<double> sum(nhel, 0.0);
-  if (p->par.precision == MG_FP64) {
-    std::vector<double> h((size_t)nprobe * nhel);
-    cudaMemcpy(h.data(), ph, sizeof(double) * h.size(), cudaMemcpyDeviceToHost);
-    for (int ih = 0; ih < nhel; ++ih) for (int64_t i = 0; i < nprobe; ++i) sum[ih] += h[(size_t)ih * nprobe + i];
-  } else {
-    std::vector<float> h((size_t)nprobe * nhel);
-    cudaMemcpy(h.data(), ph, sizeof(float) * h.size(), cudaMemcpyDeviceToHost);
-    for (int ih = 0; ih < nhel; ++ih) for (int64_t i = 0; i < nprobe; ++i) sum[ih] += h[(size_t)ih * nprobe + i];
+  std::vector<double> st(2 * nhel, 0.0);
+  if (rc == MG_OK) {
+    cudaError_t e = mg_launch_probe_stats(p->par.precision, ph, nprobe, nhel, p->stats_dev, (cudaStream_t)stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(st.data(), p->stats_dev, sizeof(double) * 2 * nhel, cudaMemcpyDeviceToHost, (cudaStream_t)stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize((cudaStream_t)stream);
+    if (e != cudaSuccess) rc = cuda_fail(e, "helicity probe statistics");
   }
   cudaFree(ph);
+  if (rc != MG_OK) return rc;
   double tot = 0;
-  for (double s : sum) tot += s;
+  for (int h = 0; h < nhel; ++h) tot += st[h];
   // reading A6: h is good iff sum_probe ME_h > eps * sum_probe sum_h ME_h
   const double eps = p->par.precision == MG_FP64 ? 1e-14 : 1e-6;
+  std::vector<char> isgood(nhel, 0);
   p->good.clear();
-  for (int ih = 0; ih < nhel; ++ih) if (sum[ih] > eps * tot) p->good.push_back(ih);
-  if (p->good.empty()) for (int ih = 0; ih < nhel; ++ih) p->good.push_back(ih);
-  MG_CUDA(cudaMemcpy(p->hel_dev, p->good.data(), sizeof(int) * p->good.size(), cudaMemcpyHostToDevice));
+  for (int h = 0; h < nhel; ++h) if (st[h] > eps * tot) { isgood[h] = 1; p->good.push_back(h); }
+  if (p->good.empty()) for (int h = 0; h < nhel; ++h) { isgood[h] = 1; p->good.push_back(h); }
+  // helicity-flip symmetry (parity invariance of QCD: |M(-h)|^2 = |M(h)|^2 event by event): where the probe batch
+  // shows it, the mirror hbar = nhel-1-h of a helicity whose top quark has lambda = +1 is not evaluated and h counts
+  // twice.  Data driven: e+ e- -> mu+ mu- (Z exchange) does not have it and keeps every good helicity.
+  const double sym = p->par.precision == MG_FP64 ? 1e-10 : 1e-4;
+  const int tpos = p->desc->npar - 3;
+  p->run.clear(); p->run_w.clear();
+  for (int h = 0; h < nhel; ++h) {
+    if (!isgood[h]) continue;
+    const int hb = nhel - 1 - h;
+    const bool paired = isgood[hb] && st[nhel + h] <= sym * (st[h] + st[hb]);
+    if (paired && !((h >> tpos) & 1)) continue;               // represented by its mirror
+    p->run.push_back(h);
+    p->run_w.push_back(paired ? 2.0 : 1.0);
+  }
+  rc = upload_helicities(p);
+  if (rc != MG_OK) return rc;
   p->probed = true;
   return MG_OK;
 }
@@ -248,11 +357,7 @@ int mg_sigma(mg_process_t* p, const void* momenta_dev, int64_t nevt, void* me_ou
     int rc = mg_helicity_probe(p, momenta_dev, nevt < 4096 ? nevt : 4096, stream);
     if (rc != MG_OK) return rc;
   }
-  { const int rc = ensure_ws(p, nevt, (int)p->good.size()); if (rc != MG_OK) return rc; }
-  p->launches = p->desc->launch(p->par.precision, (const double*)momenta_dev, me_out_dev, nevt, p->hel_dev, (int)p->good.size(),
-                  nullptr, p->pvec, p->ws, p->ws_bytes, (cudaStream_t)stream);
-  MG_CUDA(cudaGetLastError());
-  return MG_OK;
+  return run_sigma(p, momenta_dev, nevt, me_out_dev, nullptr, false, (cudaStream_t)stream);
 }
 
 int mg_sigma_host(mg_process_t* p, const void* momenta_host, int64_t nevt, void* me_out_host, void* stream) {
@@ -286,6 +391,15 @@ int mg_sigma_host(mg_process_t* p, const void* momenta_host, int64_t nevt, void*
   return MG_OK;
 }
 
+int mg_weight_max(mg_process_t* p, void* me_dev, const double* weights_dev, int64_t nevt, double* out_dev, void* stream) {
+  if (!p || !out_dev || ((!me_dev || !weights_dev) && nevt > 0)) return MG_ERR_NULL;
+  if (nevt < 0) return MG_ERR_BAD_NEVT;
+  if (((uintptr_t)me_dev & (esize(p) - 1)) || ((uintptr_t)weights_dev & 7) || ((uintptr_t)out_dev & 7)) return MG_ERR_ALIGN;
+  MG_CUDA(cudaSetDevice(p->par.device));
+  MG_CUDA(mg_launch_weight_max(p->par.precision, me_dev, weights_dev, nevt, p->wpart_dev, out_dev, (cudaStream_t)stream));
+  return MG_OK;
+}
+
 int mg_good_helicities(const mg_process_t* p, int32_t* out, int32_t capacity, int32_t* ngood) {
   if (!p || !ngood) return MG_ERR_NULL;
   *ngood = (int32_t)p->good.size();
@@ -296,34 +410,19 @@ int mg_good_helicities(const mg_process_t* p, int32_t* out, int32_t capacity, in
 int mg_process_info(const mg_process_t* p, mg_info_t* o) {
   if (!p || !o) return MG_ERR_NULL;
   const mg_procdesc_t* d = p->desc;
+  memset(o, 0, sizeof *o);
   o->npar = d->npar; o->nfinal = d->npar - 2; o->ndiagrams = d->ndiagrams; o->nhel = d->nhel;
   o->ngoodhel = (int)p->good.size(); o->ncolor = d->ncol; o->denominator = d->denominator; o->nepp = MG_NEPP;
-  o->flops_per_event_allhel = d->flops_algorithmic * d->nhel;
-  o->flops_per_event_goodhel = d->flops_algorithmic * (long long)p->good.size();
-  o->flops_executed_per_event_goodhel = d->flops_per_helicity * (long long)p->good.size();
+  o->nhel_evaluated = (int)p->run.size();
+  // per-slot work (helicity tables) is done once per (event, top helicity) that is run
+  const long long nslot = d->launch_slots ? p->ntb : 0;
+  o->flops_per_event_allhel = d->flops_algorithmic * d->nhel + d->flops_algorithmic_per_event * (d->launch_slots ? 2 : 0);
+  o->flops_per_event_goodhel = d->flops_algorithmic * (long long)p->run.size() + d->flops_algorithmic_per_event * nslot;
+  o->flops_executed_per_event_goodhel = d->flops_per_helicity * (long long)p->run.size() + d->flops_per_event * nslot;
   for (int i = 0; i < 8; ++i) o->masses[i] = p->masses[i];
   o->nkernels_per_tile = d->nkernels;
   o->launches_last_sigma = (int32_t)p->launches;
   o->workspace_bytes = (int64_t)p->ws_bytes;
-  return MG_OK;
-}
-
-int mg_fma_peak(int device, int prec, double* flops_per_s) {
-  if (!flops_per_s) return MG_ERR_NULL;
-  if (prec != MG_FP64 && prec != MG_FP32) return MG_ERR_BAD_PARAM;
-  int ndev = 0;
-  if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) { cudaGetLastError(); return MG_ERR_NO_DEVICE; }
-  MG_CUDA(cudaSetDevice(device));
-  MG_CUDA(mg_run_fma_peak(prec, flops_per_s));
-  return MG_OK;
-}
-
-int mg_dmma_peak(int device, double* flops_per_s) {
-  if (!flops_per_s) return MG_ERR_NULL;
-  int ndev = 0;
-  if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) { cudaGetLastError(); return MG_ERR_NO_DEVICE; }
-  MG_CUDA(cudaSetDevice(device));
-  MG_CUDA(mg_run_dmma_peak(flops_per_s));
   return MG_OK;
 }
 

@@ -27,38 +27,6 @@ MG_DEV void load_momentum(const double* __restrict__ mom, long long ievt, int ip
 #endif
 }
 
-// Ordered loads/stores of the per-event invariants buffer inv[item][event] (split kernel shape).  asm volatile:
-// the compiler neither hoists these out of the helicity loop nor merges repeated loads, so helicity-independent
-// operands are fetched (L1/L2) where they are used instead of living in registers or spill slots.
-#if defined(__CUDA_ARCH__) && !defined(MG_LDV_PLAIN)
-MG_DEV double ldv(const double* p) { double v; asm volatile("ld.global.ca.f64 %0, [%1];" : "=d"(v) : "l"(p)); return v; }
-MG_DEV float ldv(const float* p) { float v; asm volatile("ld.global.ca.f32 %0, [%1];" : "=f"(v) : "l"(p)); return v; }
-#else
-template <class T> MG_DEV T ldv(const T* p) { return *p; }
-#endif
-// ordered shared-memory loads (invariants staged in shared memory by a diagram-group kernel's prologue)
-#if defined(__CUDA_ARCH__)
-MG_DEV double lds(const double* p) {
-  double v; asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"((unsigned)__cvta_generic_to_shared(p))); return v;
-}
-MG_DEV float lds(const float* p) {
-  float v; asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"((unsigned)__cvta_generic_to_shared(p))); return v;
-}
-#else
-template <class T> MG_DEV T lds(const T* p) { return *p; }
-#endif
-template <class T> MG_DEV mgw::P4<T> ldps(const T* p, int blk) {
-  mgw::P4<T> o;
-#pragma unroll
-  for (int m = 0; m < 4; ++m) o.c[m] = lds(p + m * blk);
-  return o;
-}
-template <class T> MG_DEV mgw::P4<T> ldp(const T* p, long long stride) {
-  mgw::P4<T> o;
-#pragma unroll
-  for (int m = 0; m < 4; ++m) o.c[m] = ldv(p + m * stride);
-  return o;
-}
 template <class T> MG_DEV void stp(T* p, long long stride, const mgw::P4<T>& v) {
 #pragma unroll
   for (int m = 0; m < 4; ++m) p[m * stride] = v.c[m];
@@ -69,21 +37,32 @@ template <int NPAR> MG_DEV int hel_of(int h, int ipar) {
 }
 
 #ifdef __CUDACC__
+// fused shape (thread = event): loops over hel_list[0..nhel_run) and adds hel_w[ih] * |M_h|^2
 typedef int (*mg_launch_fn)(int prec, const double* mom, void* me_out, long long nevt, const int* hel_list,
-                             int nhel_run, void* perhel_out, const double* par, void* ws, size_t ws_bytes,
-                             cudaStream_t st);
+                             const double* hel_w, int nhel_run, void* perhel_out, const double* par, cudaStream_t st);
+// event-CTA shape (thread = (event, helicity)): lane_w[tb * nlane + lane] = weight of that helicity (element type of the
+// precision), ntb = number of top-quark helicities run (2: both; 1: only tb_first)
+typedef int (*mg_launch_slots_fn)(int prec, const double* mom, void* me_out, long long nevt, const void* lane_w, int ntb,
+                                  int tb_first, void* perhel_out, const double* par, void* ws, size_t ws_bytes,
+                                  cudaStream_t st);
 struct mg_procdesc_t {
   const char* proc;          // canonical process string
   int npar, ngluons, ndiagrams, nhel, ncol, denominator;
-  long long flops_per_helicity;   // generator's static count (DFMA = 2)
+  long long flops_per_helicity;   // generator's static count of what the kernels execute per evaluated helicity (DFMA = 2)
   int massive[8];            // 1 where the particle has mass mt
-  mg_launch_fn launch;
-  int ws_bytes_per_event_hel[2];  // workspace bytes per (event, helicity) for fp64 / fp32 (0: fused kernel)
-  int nkernels;              // kernel launches per event tile (diagram groups + colour + helicity sum)
+  mg_launch_fn launch;             // fused shape, else nullptr
+  mg_launch_slots_fn launch_slots; // event-CTA shape, else nullptr
+  int reserved[2];
+  int nkernels;              // kernel launches per event tile
   int has_fp32;              // fp32 kernels were generated
-  int ws_bytes_per_event[2]; // workspace bytes per event (helicity-independent invariants) for fp64 / fp32
-  long long flops_algorithmic;    // static count per helicity pass with every current computed once (no diagram-group
-                                  // recomputation): the method's own FLOPs; flops_per_helicity is what the kernels execute
+  int ws_bytes_per_event[2]; // workspace bytes per event of a tile (per-event invariants) for fp64 / fp32
+  long long flops_algorithmic;    // static count per helicity with every current computed once (no diagram-group
+                                  // recomputation): the method's own FLOPs
+  long long flops_per_event;      // executed once per (event, top-quark helicity) slot, whatever the number of
+                                  // helicities: the helicity tables (event-CTA shape)
+  long long flops_algorithmic_per_event;   // same with every table built once per slot
+  int ws_bytes_per_cta[2];   // JAMP scratch per resident CTA for fp64 / fp32
+  int nlane;                 // event-CTA shape: helicity lanes per slot = 2^(npar-1)
 };
-// mg_launch_fn returns the number of kernels it launched.
+// both launch functions return the number of kernels they launched (< 0: error).
 #endif  // __CUDACC__

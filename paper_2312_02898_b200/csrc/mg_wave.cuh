@@ -209,21 +209,6 @@ MG_DEV void cur_v3(const P4<T>& PA, const W4<T>& jA, const P4<T>& PB, const W4<T
   }
 }
 
-// Same current from helicity-independent vectors prepared once per event (split kernel shape):
-//   sdp = s (PA - PB),  sqa = s (2 PB + PA),  sqb = -s (2 PA + PB),  s = -1/(PA+PB)^2
-//   j = (jA.jB) sdp + (sqa.jA) jB + (sqb.jB) jA
-template <class T>
-MG_DEV void cur_v3p(const W4<T>& jA, const W4<T>& jB, const P4<T>& sdp, const P4<T>& sqa, const P4<T>& sqb, W4<T>& o) {
-  const C1<T> d = wdot(jA, jB);
-  const C1<T> a = pwdot(sqa, jA);
-  const C1<T> b = pwdot(sqb, jB);
-#pragma unroll
-  for (int m = 0; m < 4; ++m) {
-    o.r[m] = d.r * sdp.c[m] + a.r * jB.r[m] - a.i * jB.i[m] + b.r * jA.r[m] - b.i * jA.i[m];
-    o.i[m] = d.i * sdp.c[m] + a.r * jB.i[m] + a.i * jB.r[m] + b.r * jA.i[m] + b.i * jA.r[m];
-  }
-}
-
 // gggg kinematic structure with M in the middle:  j = s * [(A.M) C + (M.C) A - 2 (A.C) M],  s = -1/P^2.
 template <class T>
 MG_DEV void cur_k(const W4<T>& A, const W4<T>& M, const W4<T>& C, T s, W4<T>& o) {
@@ -267,7 +252,7 @@ template <class T> MG_DEV void col2(const M2<T>& m, const C1<T>& x0, const C1<T>
 }
 
 // Quark-line step from the top side (row spinor):  o = s * L jslash (qslash + m),  s = -1/(q^2-m^2).
-// quark-line steps with the helicity-independent propagator factors prepared once per event (split kernel shape):
+// quark-line steps with the helicity-independent propagator factors prepared once per event:
 //   qp = s (q0 + q3), qm = s (q0 - q3), sq1 = s q1, sq2 = s q2, ms = s m
 template <class T> MG_DEV void cur_lqp(const W4<T>& L, const W4<T>& j, T qp, T qm, T sq1, T sq2, T ms, W4<T>& o);
 template <class T> MG_DEV void cur_rqp(const W4<T>& R, const W4<T>& j, T qp, T qm, T sq1, T sq2, T ms, W4<T>& o);
@@ -322,16 +307,6 @@ MG_DEV void cur_rqp(const W4<T>& R, const W4<T>& j, T qp, T qm, T sq1, T sq2, T 
   o.i[3] = ms * tl1.i + qm * tu1.i + sq1 * tu0.i + sq2 * tu0.r;
 }
 
-// Out-of-line variants (experiment MG_NOINLINE_ROUTINES): by-value arguments and result, so that the device ABI can
-// keep them in registers; the kernel body becomes a sequence of calls and its instruction footprint shrinks.
-#if defined(__CUDACC__) && defined(MG_NOINLINE_ROUTINES)
-#define MG_NOINL __device__ __noinline__
-template <class T> MG_NOINL W4<T> nl_v3(P4<T> PA, W4<T> jA, P4<T> PB, W4<T> jB, T s) { W4<T> o; cur_v3(PA, jA, PB, jB, s, o); return o; }
-template <class T> MG_NOINL W4<T> nl_k(W4<T> A, W4<T> M, W4<T> C, T s) { W4<T> o; cur_k(A, M, C, s, o); return o; }
-template <class T> MG_NOINL W4<T> nl_lq(W4<T> L, W4<T> j, P4<T> q, T m, T s) { W4<T> o; cur_lq(L, j, q, m, s, o); return o; }
-template <class T> MG_NOINL W4<T> nl_rq(W4<T> R, W4<T> j, P4<T> q, T m, T s) { W4<T> o; cur_rq(R, j, q, m, s, o); return o; }
-#endif
-
 // ---------------------------------------------------------------------------------------------
 // K5: amplitudes.  The closing quark-gluon vertex  L jslash R = B_mu j^mu  with the bilinear
 // B_mu = L gamma_mu R (index lowered) shared by every diagram that closes on the same (L, R).
@@ -369,10 +344,6 @@ template <class T> MG_DEV C1<T> contract(const W4<T>& B, const W4<T>& j) {
   }
   return d;
 }
-
-#if defined(__CUDACC__) && defined(MG_NOINLINE_ROUTINES)
-template <class T> MG_NOINL W4<T> nl_bil(W4<T> L, W4<T> R) { W4<T> o; bilinear(L, R, o); return o; }
-#endif
 
 // Chiral halves of the bilinear (config 1, Z couplings):  BL_mu = L gamma_mu P_L R,  BR_mu = L gamma_mu P_R R
 // (P_L = upper two components in the Weyl basis); index lowered as in bilinear().

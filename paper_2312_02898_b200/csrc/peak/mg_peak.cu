@@ -1,7 +1,8 @@
-// mg_peak.cu — FMA-rate micro-benchmark: the measured denominator of "% of FP64 (FP32) peak"
-// ("DFMA micro-benchmark peak measured on the same box in the same run").
-// 16 independent FMA chains per thread, 512 threads x 4 CTAs per SM, no memory traffic in the loop.
-#include "mg_internal.h"
+// mg_peak.cu — measurement helper, NOT part of the product library: builds into libmg5b200_peak.so, which only
+// bench.py loads.  FMA-rate micro-benchmarks for the denominator of "% of FP64 (FP32) peak" ("DFMA
+// micro-benchmark peak measured on the same box in the same run"): 16 independent FMA chains per thread, 512 threads x
+// 4 CTAs per SM, no memory traffic in the loop; and the same for mma.sync.m8n8k4.f64 (DMMA.8x8x4).
+#include <cuda_runtime.h>
 
 namespace {
 template <class T>
@@ -76,7 +77,7 @@ __global__ void __launch_bounds__(256) dmma_peak_kernel(double* out, int iters, 
 }
 }  // namespace
 
-cudaError_t mg_run_dmma_peak(double* flops_per_s) {
+static cudaError_t run_dmma(double* flops_per_s) {
   int dev = 0, nsm = 0;
   cudaGetDevice(&dev);
   cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
@@ -104,6 +105,12 @@ cudaError_t mg_run_dmma_peak(double* flops_per_s) {
   return e != cudaSuccess ? e : cudaGetLastError();
 }
 
-cudaError_t mg_run_fma_peak(int prec, double* flops_per_s) {
-  return prec == 0 ? run<double>(flops_per_s) : run<float>(flops_per_s);
+// C entry points (ctypes): return 0 and the rate in FLOP/s, or a cudaError_t code.
+extern "C" int mgpeak_fma(int device, int prec, double* flops_per_s) {
+  if (cudaSetDevice(device) != cudaSuccess) return (int)cudaGetLastError();
+  return (int)(prec == 0 ? run<double>(flops_per_s) : run<float>(flops_per_s));
+}
+extern "C" int mgpeak_dmma(int device, double* flops_per_s) {
+  if (cudaSetDevice(device) != cudaSuccess) return (int)cudaGetLastError();
+  return (int)run_dmma(flops_per_s);
 }

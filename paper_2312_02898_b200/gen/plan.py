@@ -30,7 +30,6 @@ The plan is a flat list of ops in evaluation order:
    ("flush", block, a, flows)           JAMP[f] += sign*acc[block][a] for (f, sign) in flows
 Names: external gluons "e<i>", "ub" (ubar(p_t)), "vv" (v(p_t~)); internal "w<k>".
 """
-import os
 from math import factorial
 
 from . import topology as topo
@@ -93,8 +92,9 @@ def skeleton_key(skel, frontier):
 class Plan:
     """Ops for an ordered list of terms (default: all terms of the process, sorted for locality)."""
 
-    def __init__(self, n, terms=None, acc_max=6, sort=True, max_keep=0):
+    def __init__(self, n, terms=None, acc_max=6, sort=True, max_keep=0, tables=None, greedy=True):
         self.n = n
+        self.tables = tables     # tables.Tables: currents that come from the per-event helicity tables are leaves
         self.flow_index = topo.flow_index_table(n)
         self.ncol = len(self.flow_index)
         all_terms = topo.diagram_terms(n)
@@ -113,7 +113,7 @@ class Plan:
         self.lmasks = set()      # top-side quark propagators
         self.rmasks = set()      # antitop-side quark propagators
         self.blocks = {}         # block key -> dict(id, nacc, flows[a] = [(flow, sign)], last_amp_index)
-        self._build(sort)
+        self._build(sort, greedy)
 
     def _new(self):
         self._next += 1
@@ -134,6 +134,8 @@ class Plan:
         return name
 
     def g(self, tree):
+        if self.tables is not None and self.tables.has_gluon(tree):
+            return self.tables.gluon(tree)["name"]
         if tree[0] == "g":
             return "e%d" % tree[1]
         hit = self._get(("g", tree))
@@ -152,6 +154,8 @@ class Plan:
         return self._put(("g", tree), out)
 
     def l(self, chain):
+        if self.tables is not None and self.tables.has_chain(chain):
+            return self.tables.lchain(chain)["name"]
         if not chain:
             return "ub"
         hit = self._get(("l", chain))
@@ -168,6 +172,8 @@ class Plan:
         return self._put(("l", chain), out)
 
     def r(self, chain):
+        if self.tables is not None and self.tables.has_chain(chain):
+            return self.tables.rchain(chain)["name"]
         if not chain:
             return "vv"
         hit = self._get(("r", chain))
@@ -238,15 +244,15 @@ class Plan:
             out.append((blk["id"], a, sign))
         return blk, out
 
-    def _build(self, sort):
+    def _build(self, sort, greedy=True):
         keyed = []
         for term in self.terms:
             c = closure_block(term)
             keyed.append((term[:c], term[c + 1:], term[c], term))
         if sort:
             keyed.sort(key=lambda k: amp_sort_key(k[0], k[1], k[2], self.acc_max, self.n))
-            if os.environ.get("MG_GREEDY", "1") == "1":
-                keyed = _greedy_order(keyed, self.acc_max)
+            if greedy:
+                keyed = _greedy_order(keyed, self.acc_max, self.tables)
         self.namps = 0
         open_blocks = []
         for lchain, rchain, mid, term in keyed:
@@ -333,8 +339,21 @@ class Plan:
 
 
 # ------------------------------------------------------------------------------------------ amplitude order
-def _deps(key):
-    """Direct inputs (as memo keys) of an internal current; external wavefunctions are not listed."""
+def _tabled(key, tables):
+    if tables is None:
+        return False
+    if key[0] == "g":
+        return tables.has_gluon(key[1])
+    if key[0] in ("l", "r"):
+        return tables.has_chain(key[1])
+    return False
+
+
+def _deps(key, tables=None):
+    """Direct inputs (as memo keys) of an internal current; external wavefunctions and currents that come from the
+    per-event tables are not listed."""
+    if tables is not None:
+        return [d for d in _deps(key) if not _tabled(d, tables)]
     kind = key[0]
     if kind == "g":
         return [("g", c) for c in key[1][1:] if c[0] != "g"]
@@ -357,7 +376,7 @@ def _amp_accs(mid, acc_max):
     return skeleton_key(skel, frontier), combos
 
 
-def _greedy_order(keyed, acc_max):
+def _greedy_order(keyed, acc_max, tables=None):
     """Register-pressure-aware order of the amplitudes (list scheduling on the current DAG): repeatedly take the
     amplitude that adds the least live state — not-yet-computed currents (8 doubles each) and newly opened JAMP
     accumulators (2 doubles each) — net of what it lets die (currents whose consumers are all done, accumulator
@@ -368,7 +387,7 @@ def _greedy_order(keyed, acc_max):
     block_left = {}          # block key -> amplitudes still to come
     seen_nodes = set()
     for lchain, rchain, mid, term in keyed:
-        r_ = [("b", lchain, rchain)] + ([("g", mid)] if mid[0] != "g" else [])
+        r_ = [("b", lchain, rchain)] + ([("g", mid)] if mid[0] != "g" and not _tabled(("g", mid), tables) else [])
         roots.append(r_)
         clo, stack = [], list(r_)
         while stack:
@@ -376,7 +395,7 @@ def _greedy_order(keyed, acc_max):
             if k in clo:
                 continue
             clo.append(k)
-            stack.extend(_deps(k))
+            stack.extend(_deps(k, tables))
         closure.append(clo)
         sk, combos = _amp_accs(mid, acc_max)
         bkey = (lchain, rchain, sk)
@@ -388,7 +407,7 @@ def _greedy_order(keyed, acc_max):
         for k in clo:
             if k not in seen_nodes:
                 seen_nodes.add(k)
-                for d in _deps(k):
+                for d in _deps(k, tables):
                     consumers[d] = consumers.get(d, 0) + 1
     computed = set()
     open_accs = {}           # block key -> set of open accumulator ids
@@ -400,7 +419,7 @@ def _greedy_order(keyed, acc_max):
             new = [k for k in closure[i] if k not in computed]
             dec = {}
             for k in new:
-                for d in _deps(k):
+                for d in _deps(k, tables):
                     dec[d] = dec.get(d, 0) + 1
             for k in roots[i]:
                 dec[k] = dec.get(k, 0) + 1
@@ -417,7 +436,7 @@ def _greedy_order(keyed, acc_max):
         for k in closure[i]:
             if k not in computed:
                 computed.add(k)
-                for d in _deps(k):
+                for d in _deps(k, tables):
                     consumers[d] -= 1
         for k in roots[i]:
             consumers[k] -= 1
@@ -474,6 +493,17 @@ def group_key(term, n):
     if c > 0:
         return ("L", mask(term[:c])), tuple(sorted(topo.leaves_of(mid)))
     return ("R", tuple(sorted(topo.leaves_of(mid)))), mask(term[c + 1:c + 2])
+
+
+def family_key(term, n):
+    """Permutation-equivariant class of a term: (kind, gluon set).  Classes of one kind and set size are relabelings of
+    each other (emit_coop.py runs the code of one of them for all).  Kinds: "A" the (n-1)-gluon set of the closing
+    tree, "L" the gluon set on the top side of the closing block, "R" the closing block itself (terms closed on their
+    first block), "Tv3"/"Tk" the big child of the root vertex of a single-block n-gluon tree."""
+    ck, fk = group_key(term, n)
+    if ck[0] == "T":
+        return "T" + fk[0], fk[1]
+    return ck[0], ck[1]
 
 
 def amp_sort_key(lchain, rchain, mid, acc_max, n):

@@ -40,7 +40,7 @@ def test_param_struct_matches_header_and_defaults():
     p = mg.default_params()
     assert p.struct_size == C.sizeof(mg.MgParams) == 80
     assert (p.alpha_s, p.alpha_ew_inv, p.mz, p.gamma_z, p.mt, p.gamma_t) == (0.118, 132.507, 91.188, 2.4414, 173.0, 0.0)
-    assert C.sizeof(mg.MgInfo) == 8 * 4 + 2 * 8 + 8 * 8 + 2 * 4 + 8 + 8
+    assert C.sizeof(mg.MgInfo) == 8 * 4 + 2 * 8 + 8 * 8 + 2 * 4 + 8 + 8 + 2 * 4
 
 
 def test_status_strings_and_argument_errors_without_gpu():

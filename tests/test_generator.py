@@ -114,14 +114,9 @@ def test_accumulator_blocks_reproduce_term_flows_and_groups_cover_all_terms(n):
 
 def test_greedy_order_lowers_live_state_without_recomputation():
     """The register-pressure-aware amplitude order (plan._greedy_order) only permutes: same currents, same FLOPs."""
-    import os
     from paper_2312_02898_b200.gen.plan import partition_terms
     terms = [t for ph in partition_terms(4, max_terms=40, max_phase=10 ** 6)[4] for t in ph]
-    os.environ["MG_GREEDY"] = "0"
-    try:
-        a = Plan(4, terms=terms)
-    finally:
-        os.environ["MG_GREEDY"] = "1"
+    a = Plan(4, terms=terms, greedy=False)
     b = Plan(4, terms=terms)
     ca, cb = a.counts(), b.counts()
     keys = ("v3", "k", "lq", "rq", "bil", "amp")
