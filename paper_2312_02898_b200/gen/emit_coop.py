@@ -184,15 +184,16 @@ def _emit_ops(body, w, sink, sync_every):
         elif kind == "amp":
             _, b_, g, accs = op
             g = operand(g)
-            w("    const C1<T> a%d = contract(%s, %s);" % (namp, b_, g))
+            # the relabelling's sign of this amplitude (+-1, staged per visit) rides on the accumulation: FMA instead of ADD
+            w("    const C1<T> a%d = contract(%s, %s); const T s%d = ld1<T>(sgn + %du * SZ);" % (namp, b_, g, namp, namp))
             for blk, a, s in accs:
                 nm = "%d_%d" % (blk, a)
                 if nm not in declared:
                     declared.add(nm)
-                    w(" T ar%s = %sa%d.r, ai%s = %sa%d.i;" % (nm, "" if s > 0 else "-", namp, nm, "" if s > 0 else "-", namp))
+                    w(" T ar%s = %ss%d * a%d.r, ai%s = %ss%d * a%d.i;" % (nm, "" if s > 0 else "-", namp, namp, nm, "" if s > 0 else "-", namp, namp))
                 else:
                     sg = "+=" if s > 0 else "-="
-                    w(" ar%s %s a%d.r; ai%s %s a%d.i;" % (nm, sg, namp, nm, sg, namp))
+                    w(" ar%s %s s%d * a%d.r; ai%s %s s%d * a%d.i;" % (nm, sg, namp, namp, nm, sg, namp, namp))
             w("\n")
             namp += 1
         elif kind == "flush":
@@ -203,34 +204,46 @@ def _emit_ops(body, w, sink, sync_every):
 
 
 def _table_maps(local, full, pi):
-    """Per element of a body's local table layout: where the relabelled entry sits in the event-wide tables.
-    map1 / map2: index | (sign bit 30); map2 = -1 unless the relabelled current is a sum of two items."""
-    size = local.size
-    m1, m2 = [0] * size, [-1] * size
+    """For relabelling pi: per element of a body's local table layout the index of the relabelled entry in the
+    event-wide tables, and per local item the sign of the relabelled current (child swaps of ggg vertices)."""
+    m1 = [0] * local.size
+    signs = {}
     for key, it in local.items.items():
-        srcs = full.relabel(key, pi)
-        assert 1 <= len(srcs) <= 2, (key, srcs)
+        (sign, skey), = full.relabel(key, pi)
+        signs[it["name"]] = sign
         # actual particle behind each variant bit of the local item
         act = []
         for q in it["bits"]:
-            if q == 3:
-                act.append(3)
-            else:
-                g = q if q < 2 else q - 2
-                act.append(gluon_particle(pi[g]))
-        for which, (sign, skey) in enumerate(srcs):
-            src = full.items[skey]
-            assert sorted(src["bits"]) == sorted(act), (key, skey)
-            pos = [src["bits"].index(a) for a in act]
-            nv = it["nv"]
-            for c in range(8):
-                for v in range(nv):
-                    vs = 0
-                    for j, pj in enumerate(pos):
-                        vs |= ((v >> j) & 1) << pj
-                    val = (src["off"] + c * nv + vs) | ((1 << 30) if sign < 0 else 0)
-                    (m1 if which == 0 else m2)[it["off"] + c * nv + v] = val
-    return m1, m2
+            act.append(3 if q == 3 else gluon_particle(pi[q if q < 2 else q - 2]))
+        src = full.items[skey]
+        assert sorted(src["bits"]) == sorted(act), (key, skey)
+        pos = [src["bits"].index(a) for a in act]
+        nv = it["nv"]
+        for c in range(8):
+            for v in range(nv):
+                vs = 0
+                for j, pj in enumerate(pos):
+                    vs |= ((v >> j) & 1) << pj
+                m1[it["off"] + c * nv + v] = src["off"] + c * nv + vs
+    return m1, signs
+
+
+def _amp_signs(plan, item_sign):
+    """Sign of every amplitude of `plan` when its tabled operands carry the signs `item_sign` (every in-body current is a
+    single vertex, i.e. multilinear in its inputs, so signs simply multiply)."""
+    sg = dict(item_sign)
+    out = []
+    for op in plan.ops:
+        k = op[0]
+        if k == "v3":
+            sg[op[1]] = sg.get(op[2], 1) * sg.get(op[3], 1)
+        elif k == "k":
+            sg[op[1]] = sg.get(op[2], 1) * sg.get(op[3], 1) * sg.get(op[4], 1)
+        elif k in ("lq", "rq", "bil"):
+            sg[op[1]] = sg.get(op[2], 1) * sg.get(op[3], 1)
+        elif k == "amp":
+            out.append(sg.get(op[1], 1) * sg.get(op[2], 1))
+    return out
 
 
 HEADER = """// GENERATED by paper_2312_02898_b200/gen (process generator, K0) — do not edit.
@@ -244,7 +257,7 @@ using namespace mgq;
 constexpr int NPAR = %(npar)d, NGLU = %(n)d, NCOL = %(ncol)d, NHEL = %(nhel)d, NLANE = %(nlane)d, BLK = %(blk)d, SLOTS = BLK / NLANE;
 """
 
-BODY_ARGS = "unsigned sinv, unsigned tab, unsigned sj, %s* jamp, int h, int live, const int* fm"
+BODY_ARGS = "unsigned sinv, unsigned tab, unsigned sgn, unsigned sj, %s* jamp, int h, int live, const int* fm"
 
 
 def emit_coop(n, fp32=True, acc_max=24, **over):
@@ -293,12 +306,14 @@ def emit_coop(n, fp32=True, acc_max=24, **over):
     assert ninvs <= BLK, "visit_gather copies one helicity-independent operand per thread"
     ninvs += ninvs & 1
     ntabs = max(b.ntab for _, b in bodies)
-    fixed = slots * (ninvp + ninvs + ntabs) * 8
+    namps = max(b.plan.namps for _, b in bodies)
+    assert namps <= BLK
+    fixed = slots * (ninvp + ninvs) * 8 + 2 * namps * 8 + 2 * slots * ntabs * 8 + 3 * ntabs * 4
     nst_max = max(0, (cfg["smem_kb"] * 1024 - fixed) // (2 * BLK * 8))
     files, binfo = [], []
     exec_hel, exec_slot = 0, 0
     nst_used = 0
-    invmap, flowmap, tabmap1, tabmap2, bmeta = [], [], [], [], []      # flat int tables + per body offsets into them
+    invmap, flowmap, tabmap, ampsign, visits, bmeta = [], [], [], [], [], []      # flat tables + per body offsets into them
     for bi, (fi, b) in enumerate(bodies):
         fam = fams[fi]
         nm_ = len(fam["members"])
@@ -336,8 +351,8 @@ def emit_coop(n, fp32=True, acc_max=24, **over):
                              what="body %d of %d (family %s%d, executed for %d relabellings per visit)"
                                   % (bi, nbody, fam["kind"], fam["size"], nm_))]
         o = out.append
-        o("template <class T>\nMG_DEV void body%d_impl(const unsigned sinv, const unsigned tab, const unsigned sj, T* __restrict__ jamp,\n"
-          "                      const int h, const int live, const int* __restrict__ fm) {\n" % bi)
+        o("template <class T>\nMG_DEV void body%d_impl(const unsigned sinv, const unsigned tab, const unsigned sgn, const unsigned sj,\n"
+          "                      T* __restrict__ jamp, const int h, const int live, const int* __restrict__ fm) {\n" % bi)
         o("  constexpr unsigned SZ = (unsigned)sizeof(T), COL = (unsigned)BLK * SZ;\n")
         for bits, nm in sorted(vaddr.items()):
             if bits:
@@ -353,25 +368,26 @@ def emit_coop(n, fp32=True, acc_max=24, **over):
                   % (b.slot[f], 2 * sl, 2 * sl + 1))
             o("  }\n")
         o("}\n")
-        o("__device__ __noinline__ void body%d(%s) {\n  body%d_impl<double>(sinv, tab, sj, jamp, h, live, fm);\n}\n"
+        o("__device__ __noinline__ void body%d(%s) {\n  body%d_impl<double>(sinv, tab, sgn, sj, jamp, h, live, fm);\n}\n"
           % (bi, BODY_ARGS % "double", bi))
         if fp32:
-            o("__device__ __noinline__ void body%d(%s) {\n  body%d_impl<float>(sinv, tab, sj, jamp, h, live, fm);\n}\n"
+            o("__device__ __noinline__ void body%d(%s) {\n  body%d_impl<float>(sinv, tab, sgn, sj, jamp, h, live, fm);\n}\n"
               % (bi, BODY_ARGS % "float", bi))
         o("}  // namespace\n")
         files.append(("%s_b%02d.cu" % (ns, bi), "".join(out)))
         # per member: gather map of the helicity-independent operands, colour-flow map
-        bmeta.append((len(invmap), len(flowmap), len(tabmap1)))
+        bmeta.append((len(flowmap), len(visits)))
         for pi in fam["members"]:
+            visits.append((len(tabmap), b.ntab, len(invmap), b.ninv, len(ampsign), b.plan.namps))
             for nm, off in sorted(b.inv.items(), key=lambda kv: kv[1]):
                 src = inv[_perm_name(nm, pi)]
                 invmap += [src + j for j in range(b.sizes[nm])]
             for f in b.flows:
                 o_ = tuple(pi[g] for g in flow_order[f])
                 flowmap.append(2 * flow_index[o_] * BLK)
-            m1, m2 = _table_maps(b.tables, ftab, pi)
-            tabmap1 += m1
-            tabmap2 += m2
+            m1, isign = _table_maps(b.tables, ftab, pi)
+            tabmap += m1
+            ampsign += _amp_signs(b.plan, isign)
         binfo.append(dict(family="%s%d" % (fam["kind"], fam["size"]), members=nm_, terms=len(b.plan.terms), flops=flops,
                           flows=len(touches), staged=len(staged), max_live=b.plan.max_live(), ninv=b.ninv, ntab=b.ntab))
     colour_flops = 2 * (ncol * (ncol - 1) // 2) * 2 + ncol * 8
@@ -380,9 +396,9 @@ def emit_coop(n, fp32=True, acc_max=24, **over):
     algo_slot = gt.flops()           # the tabled currents the diagrams actually use, once per slot
     exec_slot = ftab.flops()         # the kernel builds every current the thresholds allow
     smem = fixed + 2 * nst_used * BLK * 8
-    files.append(_main_unit(E, n, ns, hdr, cfi, cfden, fams, bodies, bmeta, invmap, flowmap, (tabmap1, tabmap2), ftab, ntabf, inv,
-                            ninv, ninvp, ninvs, ntabs, nst_used, fp32, exec_hel + colour_flops, algo + colour_flops, exec_slot,
-                            algo_slot, cfg))
+    files.append(_main_unit(E, n, ns, hdr, cfi, cfden, fams, bodies, bmeta, invmap, flowmap, (tabmap, ampsign, visits, namps), ftab,
+                            ntabf, inv, ninv, ninvp, ninvs, ntabs, nst_used, fp32, exec_hel + colour_flops, algo + colour_flops,
+                            exec_slot, algo_slot, cfg))
     info = dict(proc=proc, ns=ns, npar=npar, ncol=ncol, nhel=nhel, ndiagrams=ndiag,
                 nterms=sum(len(b.plan.terms) * len(fams[fi]["members"]) for fi, b in bodies),
                 flops_per_helicity=exec_hel + colour_flops, flops_algorithmic=algo + colour_flops, flops_per_slot=exec_slot,
@@ -416,12 +432,24 @@ def _main_unit(E, n, ns, hdr, cfi, cfden, fams, bodies, bmeta, invmap, flowmap, 
 
     table("inv_map", "short", invmap)
     table("flow_map", "int", flowmap, 16)
-    w("__device__ const int2 tab_map[%d] = {\n" % max(1, len(tabmaps[0])))
-    for k_ in range(0, len(tabmaps[0]), 8):
-        w("  " + ", ".join("{%d, %d}" % (a_, b_) for a_, b_ in zip(tabmaps[0][k_:k_ + 8], tabmaps[1][k_:k_ + 8])) + ",\n")
-    if not tabmaps[0]:
-        w("  {0, -1}\n")
+    tabmap, ampsign, visits, namps = tabmaps
+    table("tab_map", "int", tabmap, 24)
+    w("__device__ const double amp_sign64[%d] = {\n" % max(1, len(ampsign)))
+    for k_ in range(0, len(ampsign), 40):
+        w("  " + ", ".join("%d." % v for v in ampsign[k_:k_ + 40]) + ",\n")
     w("};\n")
+    if fp32:
+        w("__device__ const float amp_sign32[%d] = {\n" % max(1, len(ampsign)))
+        for k_ in range(0, len(ampsign), 40):
+            w("  " + ", ".join("%d.f" % v for v in ampsign[k_:k_ + 40]) + ",\n")
+        w("};\n")
+        w("MG_DEV const float* amp_sign_of(float*) { return amp_sign32; }\n")
+    w("MG_DEV const double* amp_sign_of(double*) { return amp_sign64; }\n")
+    w("constexpr int NVISIT = %d, NAMPS = %d;\n" % (len(visits), namps))
+    w("__device__ const VisitDesc visit_desc[NVISIT + 2] = {\n")
+    for v_ in visits:
+        w("  {%d, %d, %d, %d, %d, %d, 0, 0},\n" % v_)
+    w("  {0, 0, 0, 0, 0, 0, 0, 0}, {0, 0, 0, 0, 0, 0, 0, 0}};\n")
     # helicity-bit shifts per family member: canonical gluon i takes the helicity of gluon pi[i]
     hsh, foff_of = [], {}
     for fi, fam in enumerate(fams):
@@ -510,16 +538,16 @@ def _main_unit(E, n, ns, hdr, cfi, cfden, fams, bodies, bmeta, invmap, flowmap, 
     calls = []
     for bi, (fi, b) in enumerate(bodies):
         nm_ = len(fams[fi]["members"])
-        io, fo, to = bmeta[bi]
+        fo, v0 = bmeta[bi]
         calls.append(
             "    // body %d: family %s%d, %d terms, %d relabellings\n"
             "#pragma unroll 1\n    for (int m = 0; m < %d; ++m) {\n"
-            "      visit_gather<T, SLOTS>(sinv0, sinvp0, tabp0, gtab, inv_map + %d + m * %d, %d, tab_map + %d + m * %d, %d,\n"
-            "                             NINVP, NINVS, NTABS, NTABF);\n"
+            "      const int v = %d + m;\n"
+            "      visit_step<T, SLOTS>(visit_desc, v, tab_map, inv_map, gtab, asgn, sinv0, sinvp0, smap0, stab0, ssgn0, NINVP, NINVS, NTABS, NTABF, NAMPS);\n"
             "      const int hp = permute_helicity<NPAR, NGLU>(h, hel_shift + %d + m * NGLU);\n"
-            "      body%d(sinvp, tabp, sj, jamp, hp, live, flow_map + %d + m * %d);\n    }\n"
-            % (bi, fams[fi]["kind"], fams[fi]["size"], len(b.plan.terms), nm_, nm_, io, b.ninv, b.ninv, to, b.ntab, b.ntab,
-               foff_of[fi], bi, fo, len(b.flows)))
+            "      body%d(sinvp, stab0 + (unsigned)(((v & 1) * SLOTS + slot) * NTABS) * SZ, ssgn0 + (unsigned)((v & 1) * NAMPS) * SZ, sj, jamp, hp, live,\n"
+            "             flow_map + %d + m * %d);\n    }\n"
+            % (bi, fams[fi]["kind"], fams[fi]["size"], len(b.plan.terms), nm_, nm_, v0, foff_of[fi], bi, fo, len(b.flows)))
     w(KERNEL % dict(calls="".join(calls),
                     colour=("colour_dmma_cta<NCOL, BLK>(cf_dense, (const double*)jamp_cta, reinterpret_cast<double*>(smem_raw), (double*)s_meh);\n"
                             "    T meh = s_meh[tid];" if dmma else
@@ -560,10 +588,13 @@ sigma_kernel(long long nevt, int ntb, int tb_first, const T* __restrict__ lane_w
   constexpr unsigned SZ = (unsigned)sizeof(T);
   const unsigned sbase = (unsigned)__cvta_generic_to_shared(smem_raw);
   const int tid = threadIdx.x, slot = tid / NLANE, lane = tid %% NLANE;
-  // shared memory: full per-event operand set | the running body's operand subset | its helicity tables | staged JAMPs
-  const unsigned sinv0 = sbase, sinvp0 = sinv0 + SLOTS * NINVP * SZ, tabp0 = sinvp0 + SLOTS * NINVS * SZ;
-  const unsigned sj = tabp0 + SLOTS * NTABS * SZ + tid * SZ;
-  const unsigned sinvp = sinvp0 + slot * NINVS * SZ, tabp = tabp0 + slot * NTABS * SZ;
+  // shared memory: full per-event operand set | the running visit's helicity-independent operands | amplitude signs [2] |
+  // table operands [2] | index maps [3] | staged JAMPs
+  const unsigned sinv0 = sbase, sinvp0 = sinv0 + SLOTS * NINVP * SZ, ssgn0 = sinvp0 + SLOTS * NINVS * SZ;
+  const unsigned stab0 = ssgn0 + 2 * NAMPS * SZ, smap0 = stab0 + 2 * SLOTS * NTABS * SZ;
+  const unsigned sj = smap0 + 3 * NTABS * 4 + ((NTABS & 1) ? 4 : 0) + tid * SZ;
+  const unsigned sinvp = sinvp0 + slot * NINVS * SZ;
+  const T* __restrict__ asgn = amp_sign_of((T*)nullptr);
   T* __restrict__ sinv_g = reinterpret_cast<T*>(smem_raw);
   T* __restrict__ jamp_cta = scratch + (size_t)blockIdx.x * (2 * NCOL * BLK + SLOTS * NTABF);
   T* __restrict__ jamp = jamp_cta + tid;
@@ -589,7 +620,9 @@ sigma_kernel(long long nevt, int ntb, int tb_first, const T* __restrict__ lane_w
     const int live = slot_live && wgt != T(0);
     __syncthreads();
     build_tables_global<T>(tab_groups, NGROUPS, tab_desc, sinv0, gtab, NINVP, NTABF, SLOTS, s_tbit);
+    visit_prologue<T, SLOTS>(visit_desc, tab_map, gtab, asgn, smap0, stab0, ssgn0, NTABS, NTABF, NAMPS);
 %(calls)s
+    visit_drain();
     __threadfence();                       // the JAMP reductions are performed at L2 before anyone reads them back
     __syncthreads();
     %(colour)s
@@ -619,7 +652,7 @@ static int run(const double* mom, T* me_out, long long nevt, const T* lane_w, in
   norm /= (double)%(cfden)d * (double)%(denom)d;
   int dev = 0, nsm = 0, per_sm = 0;
   if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return -1;
-  size_t smem = (size_t)(SLOTS * (NINVP + NINVS + NTABS) + 2 * NST * BLK) * sizeof(T);
+  size_t smem = (size_t)(SLOTS * (NINVP + NINVS) + 2 * NAMPS + 2 * SLOTS * NTABS + 2 * NST * BLK) * sizeof(T) + 3 * NTABS * 4 + 8;
   if (sizeof(T) == 8 && smem < COLOUR_SMEM) smem = COLOUR_SMEM;
   auto kern = sigma_kernel<T>;
   if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return -1;

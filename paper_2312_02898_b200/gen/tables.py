@@ -17,7 +17,7 @@ it is fixed while a table is alive (half the top-side chain tables, and a run th
 """
 from . import topology as topo
 
-KIND = {"eg": 0, "q": 1, "v3": 2, "k": 3, "lq": 4, "rq": 5}
+KIND = {"eg": 0, "q": 1, "v3": 2, "k": 3, "lq": 4, "rq": 5, "kz": 6}
 
 
 def gluon_particle(i):
@@ -63,9 +63,16 @@ class Tables:
         key = ("g", tree)
         if key in self.items:
             return self.items[key]
-        kids = [self.gluon(c) for c in tree[1:]]
         leaves = sorted(topo.leaves_of(tree))
         mask = topo.leafmask(tree)
+        if tree[0] == "kz":
+            # the eliminated four-gluon structure K_Z = -K_X - K_Y (parts x, y, z by smallest leaf), kept in the
+            # event-wide tables so that every relabelled entry is a plain copy of one item
+            x, y, z = tree[1:]
+            kids = [self.gluon(("k", y, x, z)), self.gluon(("k", x, y, z))]
+            return self._add(key, "kz", [gluon_particle(i) for i in leaves], [k["key"] for k in kids], [], len(leaves),
+                             "tg%d" % len(self.items))
+        kids = [self.gluon(c) for c in tree[1:]]
         if tree[0] == "v3":
             inv = ["pm%d" % topo.leafmask(tree[1]), "pm%d" % topo.leafmask(tree[2]), "sg%d" % mask]
         else:
@@ -141,7 +148,7 @@ class Tables:
     def flops(self):
         """Static FLOPs of building all tables once (per event)."""
         from .plan import FLOPS
-        cost = {"v3": FLOPS["v3"], "k": FLOPS["k"], "lq": FLOPS["lq"], "rq": FLOPS["rq"], "eg": 0, "q": 0}
+        cost = {"v3": FLOPS["v3"], "k": FLOPS["k"], "lq": FLOPS["lq"], "rq": FLOPS["rq"], "eg": 0, "q": 0, "kz": 8}
         return sum(cost[it["kind"]] * it["nv"] for it in self.items.values())
 
     def inv_names(self):
@@ -163,6 +170,8 @@ class Tables:
             for S in combinations(gl, k):
                 for t in topo.gluon_tree_terms(S):
                     self.gluon(t)
+                    if t[0] == "k" and min(topo.leaves_of(t[1])) < min(topo.leaves_of(t[2])):     # the K_Y term: parts in order
+                        self.gluon(("kz", t[1], t[2], t[3]))
         for k in range(1, self.qtab + 1):
             for S in combinations(gl, k):
                 for blocks in topo.ordered_block_partitions(S):
@@ -203,7 +212,7 @@ class Tables:
 def relabel_tree(tree, pi):
     """Tree with every leaf i replaced by pi[i], brought to the canonical embedding of topology.gluon_tree_terms
     (children of a ggg vertex ordered by smallest leaf: a swap costs a sign; a gggg structure whose middle part is the
-    one with the largest smallest-leaf is K_Z = -K_X - K_Y).  Returns [(sign, canonical tree)]."""
+    one with the largest smallest-leaf is the "kz" item K_Z = -K_X - K_Y).  Returns [(sign, canonical tree)]."""
     if tree[0] == "g":
         return [(1, ("g", pi[tree[1]]))]
     kids = [relabel_tree(c, pi) for c in tree[1:]]
@@ -226,6 +235,5 @@ def relabel_tree(tree, pi):
                 elif m is y:
                     out.append((s, ("k", x, y, z)))
                 else:
-                    out.append((-s, ("k", y, x, z)))
-                    out.append((-s, ("k", x, y, z)))
+                    out.append((s, ("kz", x, y, z)))
     return out
