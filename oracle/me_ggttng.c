@@ -128,9 +128,8 @@ static void setup_externals(bg_t* b, int nfinal, const double* p, const oracle_p
 static double me_c4(int nfinal, const double* p, const oracle_params_t* par, double* hel_out, int ward_which) {
   int n = 2 + nfinal, npar = n + 2, nhel = 1 << npar;
   if (n < 2 || n > 5) return -1;
-  static int perms[120][5];
-  #pragma omp critical(oracle_perms)
-  { oracle_all_perms(n, perms); }
+  int perms[120][5];               /* per call (threads of oracle_me_batch each fill their own copy) */
+  oracle_all_perms(n, perms);
   int np = 1; for (int i = 2; i <= n; ++i) np *= i;
   const double* CF = colour_matrix_cached(n);
   real denom = 256; for (int i = 2; i <= nfinal; ++i) denom *= i;     /* 2*2*8*8*(n-2)!  (A3) */

@@ -92,4 +92,9 @@ double oracle_me_ggttng_ward(int nfinal_gluons, const double* p, const oracle_pa
 int oracle_me_batch(int proc, const double* momenta, int64_t nevt, const oracle_params_t* par,
                     double* me_out, int nthreads);
 int oracle_num_threads(void);
+
+/* ---- batch-unweighting primitive (PAPER.md:99-:103): prod_i = w_i * me_i rounded once to double (single != 0: to
+ * float), out3 = (max_i, sum_i, sum_i prod_i^2) of the products; prod_out may be NULL.  Pinned by closed forms
+ * (arithmetic series) and by the exactness of the maximum (tests/test_oracle_weight.py). ---- */
+int oracle_weight_max(const double* me, const double* w, int64_t n, int single, double* prod_out, double* out3);
 #endif

@@ -56,6 +56,7 @@ class Oracle:
         L.oracle_me_ggttng_ward.restype = C.c_double
         L.oracle_rambo.argtypes = [C.c_uint64, C.c_int64, C.c_int64, C.c_int, _dp, C.c_double, _dp, _dp]
         L.oracle_me_batch.argtypes = [C.c_int, _dp, C.c_int64, C.POINTER(Params), _dp, C.c_int]
+        L.oracle_weight_max.argtypes = [_dp, _dp, C.c_int64, C.c_int, _dp, _dp]
 
     def philox(self, ctr, key):
         c = (C.c_uint32 * 4)(*ctr); k = (C.c_uint32 * 2)(*key); o = (C.c_uint32 * 4)()
@@ -130,6 +131,13 @@ class Oracle:
         rc = self.lib.oracle_me_batch(ip, _p(mom), mom.shape[0], C.byref(par), _p(out), nthreads)
         assert rc == 0
         return out
+
+    def weight_max(self, me, w, single=False):
+        """(products, (max, sum, sum of squares)) of w * me."""
+        me = np.ascontiguousarray(me, dtype=np.float64); w = np.ascontiguousarray(w, dtype=np.float64)
+        prod = np.zeros(len(me)); out = np.zeros(3)
+        self.lib.oracle_weight_max(_p(me), _p(w), len(me), 1 if single else 0, _p(prod), _p(out))
+        return prod, out
 
     def num_threads(self):
         return int(self.lib.oracle_num_threads())

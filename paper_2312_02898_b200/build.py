@@ -88,7 +88,12 @@ def _compile(path, force, log):
     stamp = _stamp(path)
     if not force and os.path.exists(obj) and os.path.exists(stamp_file) and open(stamp_file).read() == stamp:
         return obj
-    cmd = [NVCC] + ARCH + FLAGS + ["-Xptxas", "-v", "-c", path, "-o", obj]
+    extra = []
+    with open(path) as fh:                      # per-unit flags requested by the generator ("// nvcc: ..." in the header)
+        for line in fh.readlines()[:4]:
+            if line.startswith("// nvcc:"):
+                extra = line[len("// nvcc:"):].split()
+    cmd = [NVCC] + ARCH + FLAGS + extra + ["-Xptxas", "-v", "-c", path, "-o", obj]
     r = subprocess.run(cmd, capture_output=True, text=True)
     with open(os.path.join(OBJ, base + ".ptxas.log"), "w") as fh:
         fh.write(" ".join(cmd) + "\n" + r.stdout + r.stderr)

@@ -246,7 +246,7 @@ def _amp_signs(plan, item_sign):
     return out
 
 
-HEADER = """// GENERATED by paper_2312_02898_b200/gen (process generator, K0) — do not edit.
+HEADER = """// GENERATED by paper_2312_02898_b200/gen (process generator, K0) — do not edit.%(nvcc)s
 // process: %(proc)s   gluons: %(n)d   Feynman diagrams: %(ndiag)d (whole process)
 // this unit: %(what)s
 // diagram terms here: %(nterms)d   colour flows: %(ncol)d   helicities: %(nhel)d   static flops / helicity here: %(flops)d
@@ -280,7 +280,10 @@ def emit_coop(n, fp32=True, acc_max=24, **over):
     flow_index = topo.flow_index_table(n)
     flow_order = {i: p for p, i in flow_index.items()}
     fams = families(n, cfg["max_phase"])
-    hdr = dict(proc=proc, n=n, ncol=ncol, nhel=nhel, ns=ns, npar=npar, nlane=nlane, blk=BLK)
+    # bodies are compiled for the register budget of the kernel's occupancy target (build.py reads the "nvcc:" line)
+    maxreg = min(255, 65536 // (BLK * cfg.get("ctas_per_sm", 256 // BLK)) // 8 * 8)
+    hdr = dict(proc=proc, n=n, ncol=ncol, nhel=nhel, ns=ns, npar=npar, nlane=nlane, blk=BLK,
+               nvcc="\n// nvcc: -maxrregcount=%d" % maxreg if maxreg < 255 else "")
     bodies = []                  # (family index, _Body)
     for fi, fam in enumerate(fams):
         for terms in fam["bodies"]:
@@ -446,7 +449,7 @@ def _main_unit(E, n, ns, hdr, cfi, cfden, fams, bodies, bmeta, invmap, flowmap, 
         w("MG_DEV const float* amp_sign_of(float*) { return amp_sign32; }\n")
     w("MG_DEV const double* amp_sign_of(double*) { return amp_sign64; }\n")
     w("constexpr int NVISIT = %d, NAMPS = %d;\n" % (len(visits), namps))
-    w("__device__ const VisitDesc visit_desc[NVISIT + 2] = {\n")
+    w("__constant__ VisitDesc visit_desc[NVISIT + 2] = {\n")
     for v_ in visits:
         w("  {%d, %d, %d, %d, %d, %d, 0, 0},\n" % v_)
     w("  {0, 0, 0, 0, 0, 0, 0, 0}, {0, 0, 0, 0, 0, 0, 0, 0}};\n")
@@ -548,7 +551,7 @@ def _main_unit(E, n, ns, hdr, cfi, cfden, fams, bodies, bmeta, invmap, flowmap, 
             "      body%d(sinvp, stab0 + (unsigned)(((v & 1) * SLOTS + slot) * NTABS) * SZ, ssgn0 + (unsigned)((v & 1) * NAMPS) * SZ, sj, jamp, hp, live,\n"
             "             flow_map + %d + m * %d);\n    }\n"
             % (bi, fams[fi]["kind"], fams[fi]["size"], len(b.plan.terms), nm_, nm_, v0, foff_of[fi], bi, fo, len(b.flows)))
-    w(KERNEL % dict(calls="".join(calls),
+    w(KERNEL % dict(calls="".join(calls), minb=cfg.get("ctas_per_sm", 256 // BLK),
                     colour=("colour_dmma_cta<NCOL, BLK>(cf_dense, (const double*)jamp_cta, reinterpret_cast<double*>(smem_raw), (double*)s_meh);\n"
                             "    T meh = s_meh[tid];" if dmma else
                             "T meh = colour_reg<T>(jamp);"),
@@ -578,7 +581,7 @@ KERNEL = """
 // particles.  ntb = number of top helicities run (2: both, slots 2k / 2k+1 are lambda_t = -1 / +1 of event k;
 // 1: only tb_first — the helicity-flip symmetry |M(-h)|^2 = |M(h)|^2 is in the lane weights, mg_api.cu).
 template <class T>
-__global__ void __launch_bounds__(BLK, 256 / BLK)
+__global__ void __launch_bounds__(BLK, %(minb)d)
 sigma_kernel(long long nevt, int ntb, int tb_first, const T* __restrict__ lane_w, const T* __restrict__ invbuf,
              T* __restrict__ scratch, T* __restrict__ me_out, T* __restrict__ perhel_out,
              long long perhel_stride, T norm) {
@@ -657,7 +660,7 @@ static int run(const double* mom, T* me_out, long long nevt, const T* lane_w, in
   auto kern = sigma_kernel<T>;
   if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return -1;
   if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, BLK, smem) != cudaSuccess || per_sm < 1) return -1;
-  if (per_sm > 2) per_sm = 2;                             // mg_api.cu sizes the scratch for at most 2 CTAs per SM
+  if (per_sm > 4) per_sm = 4;                             // mg_api.cu sizes the scratch for at most 4 CTAs per SM
   const long long ncta_max = (long long)per_sm * nsm;
   const size_t per_cta = (size_t)2 * NCOL * BLK + (size_t)SLOTS * NTABF;
   const size_t scratch_bytes = (size_t)ncta_max * per_cta * sizeof(T);

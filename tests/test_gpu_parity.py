@@ -1,10 +1,14 @@
 """GPU parity tests: the CUDA path, called through the C ABI (paper_2312_02898_b200 binding), against the
 CPU oracle on identical seeded inputs (SURVEY.md §8c "parity protocol").
 
-  * Philox words: bit-exact.   * RAMBO momenta: <= 1e-12 sqrt(s) per component (libm differs).
-  * |M|^2 fp64: relative 1e-10 per event vs the long-double oracle on the GPU-generated momenta.
+  * Philox words: bit-exact.
+  * RAMBO momenta: adjudicated against the long-double oracle — the CUDA sampler must be as close to it as the
+    double oracle is (libm log/sincos differ by an ulp, the conformal boost amplifies that for collinear q's).
+  * |M|^2 fp64: per event  rel <= max(1e-10, C 2^-53 s / (2 min_ij |p_i.p_j|))  against the long-double oracle on the
+    GPU-generated momenta (north_star's 1e-10, and a conditioning allowance near soft/collinear poles whose constant
+    C = 16 is ten times what the oracle's own double build needs there: DESIGN.md §3, reading A12).
   * |M|^2 fp32: median 1e-5, max 1e-3 (north_star).
-All tests need a CUDA device (-m gpu).
+All tests need a CUDA device (-m gpu).  `--full-parity` runs the whole SURVEY.md §8(d) parity set for gg -> tt~ggg too.
 """
 import math
 
@@ -17,6 +21,37 @@ pytestmark = pytest.mark.gpu
 
 TOL64 = 1e-10           # north_star
 TOL32_MED, TOL32_MAX = 1e-5, 1e-3
+COND_C = 16.0           # conditioning allowance: rel <= max(TOL64, COND_C * 2^-53 * s / (2 min |p_i.p_j|))
+
+
+def min_gluon_invariant(ev):
+    """min over pairs of massless legs (gluons) of |p_i.p_j|: the soft / collinear poles of gg -> tt~ + gluons."""
+    npar = ev.shape[1]
+    out = np.full(len(ev), np.inf)
+    glu = [a for a in range(npar) if a not in (2, 3)]
+    for i, a in enumerate(glu):
+        for b in glu[i + 1:]:
+            d = ev[:, a, 0] * ev[:, b, 0] - (ev[:, a, 1:] * ev[:, b, 1:]).sum(-1)
+            out = np.minimum(out, np.abs(d))
+    return out
+
+
+def parity_bound(ev, sqrt_s):
+    return np.maximum(TOL64, COND_C * 2.0 ** -53 * sqrt_s ** 2 / (2.0 * min_gluon_invariant(ev)))
+
+
+def report(tag, rel, bound):
+    """A12 report: median, 99.9 %, max, count above 1e-10 (and above the per-event bound); kept in gpurun_out/ if present."""
+    import json
+    import os
+    rec = dict(case=tag, n=int(len(rel)), median=float(np.median(rel)), q999=float(np.quantile(rel, 0.999)), max=float(rel.max()),
+               above_1e10=int((rel > TOL64).sum()), above_bound=int((rel > bound).sum()))
+    print("parity", rec)
+    out = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "gpurun_out")
+    if os.path.isdir(out):
+        with open(os.path.join(out, "parity_report.jsonl"), "a") as fh:
+            fh.write(json.dumps(rec) + "\n")
+    return rec
 
 
 @pytest.fixture(scope="module")
@@ -60,7 +95,7 @@ def test_philox_words_bit_exact(mg, oracle):
 
 
 @pytest.mark.parametrize("name", ["eemumu", "ggtt", "ggttg", "ggttgg", "ggttggg"])
-def test_rambo_matches_oracle_and_invariants(mg, oracle, name):
+def test_rambo_matches_oracle_and_invariants(mg, oracle, oracle_ld, name):
     cfg = workloads.CONFIGS[name]
     if not available(mg, name):
         pytest.skip("process not generated")
@@ -68,10 +103,14 @@ def test_rambo_matches_oracle_and_invariants(mg, oracle, name):
     nevt = 4133                      # several pages + ragged tail
     mom, ev = gpu_events(mg, proc, cfg, nevt)
     ref = oracle.rambo(cfg["seed"], nevt, cfg["masses_final"], cfg["sqrt_s"])
-    # libm log/sincos differ by an ulp between glibc and CUDA; RAMBO's conformal boost amplifies that by
-    # (Q0/M)^2 for nearly collinear massless q's, so the bound is on quantiles, with a loose cap
-    dev = np.abs(ev - ref).reshape(nevt, -1).max(axis=1) / cfg["sqrt_s"]
-    assert np.median(dev) <= 1e-14 and np.quantile(dev, 0.99) <= 1e-12 and dev.max() <= 1e-9, (np.median(dev), dev.max())
+    refl = oracle_ld.rambo(cfg["seed"], nevt, cfg["masses_final"], cfg["sqrt_s"])
+    # libm log/sincos differ by an ulp between glibc and CUDA, and RAMBO's conformal boost amplifies rounding by
+    # (Q0/M)^2 for nearly collinear massless q's: no flat bound holds.  Adjudication: per event, the CUDA sampler may
+    # deviate from the long-double oracle by at most 4x what the double oracle itself deviates (plus one ulp of sqrt(s))
+    dev = np.abs(ev - refl).reshape(nevt, -1).max(axis=1) / cfg["sqrt_s"]
+    own = np.abs(ref - refl).reshape(nevt, -1).max(axis=1) / cfg["sqrt_s"]
+    assert np.all(dev <= 4 * own + 8 * 2.0 ** -53), (float((dev / (own + 2.0 ** -53)).max()), float(dev.max()))
+    assert np.median(dev) <= 1e-15
     # weights and first_event offset (sharded call gives the same events)
     import torch
     mom2, w2 = proc.rambo(cfg["seed"], cfg["sqrt_s"], 100, first_event=4000, weights=True)
@@ -117,13 +156,18 @@ def test_sigma_fp64_parity_small(mg, oracle, oracle_ld, name):
         proc.close()
 
 
+# SURVEY.md §8(d) parity set on BASELINE.json's full batches, in the launch configuration bench.py times: (first N events,
+# the H events of the full batch with the smallest gluon invariants = numerically hardest).  The long-double oracle
+# adjudicates everything except the bulk of gg -> tt~ggg, where it costs 0.1 s per event: there the double oracle is the
+# reference for the first N events (its own error on such events is < 1e-12, measured against the long-double build)
+# and the long-double one for the hardest H.
+PARITY_SET = {"eemumu": (16384, 0), "ggtt": (524288, 0), "ggttg": (65536, 1024), "ggttgg": (16384, 1024), "ggttggg": (2048, 128)}
+PARITY_SET_FULL = {"ggttg": (524288, 1024), "ggttggg": (16384, 1024)}
+
+
 @pytest.mark.parametrize("name", ["eemumu", "ggtt", "ggttg", "ggttgg", "ggttggg"])
-def test_sigma_fp64_full_size_sampled(mg, oracle, oracle_ld, name):
-    """BASELINE.json's full sizes, in the launch configuration bench.py times: sampled events are
-    checked one by one against the oracle (plus the numerically hardest ones: smallest min s_ij)."""
+def test_sigma_fp64_parity_set_full_batch(mg, oracle, oracle_ld, full_parity, name):
     cfg = workloads.CONFIGS[name]
-    if not available(mg, name):
-        pytest.skip("process not generated")
     import torch
     nevt = cfg["nevt"]
     proc = mg.Process(cfg["proc"])
@@ -132,31 +176,27 @@ def test_sigma_fp64_full_size_sampled(mg, oracle, oracle_ld, name):
     torch.cuda.synchronize()
     me = me.cpu().numpy()
     assert np.all(np.isfinite(me)) and np.all(me > 0)
-    nsamp = {"eemumu": 2048, "ggtt": 2048, "ggttg": 1024, "ggttgg": 256, "ggttggg": 12}[name]
-    rng = np.random.default_rng(12345)
-    idx = rng.choice(nevt, size=nsamp, replace=False)
-    idx[:3] = [0, nevt - 1, nevt // 2]
-    orc = oracle_ld
-    ref = orc.me_batch(cfg["proc"], ev[idx])
+    nfirst, nhard = (PARITY_SET_FULL if full_parity else {}).get(name, PARITY_SET[name])
+    bulk = oracle if name == "ggttggg" else oracle_ld
+    idx = np.arange(nfirst)
+    ref = bulk.me_batch(cfg["proc"], ev[idx])
     rel = np.abs(me[idx] / ref - 1)
-    assert np.median(rel) < 1e-12 and rel.max() < TOL64, (rel.max(), np.median(rel))
-    if name.startswith("ggttg"):
-        # the numerically hardest events of the batch (smallest invariants: soft / collinear gluons).  Both sides
-        # are given the same doubles, but near a soft or collinear pole |M|^2 is ill-conditioned in them: the fp64
-        # result carries rounding amplified by ~ s / min s_ij (reading A12), so the bound is a
-        # conditioning cap: median 1e-9, max 1e-8 over the hardest events of the batch.
-        npar = ev.shape[1]
-        smin = np.full(nevt, np.inf)
-        for a in range(npar):
-            for b in range(a + 1, npar):
-                if a in (2, 3) and b in (2, 3):
-                    continue
-                d = ev[:, a, 0] * ev[:, b, 0] - (ev[:, a, 1:] * ev[:, b, 1:]).sum(-1)
-                smin = np.minimum(smin, np.abs(d))
-        hard = np.argsort(smin)[: max(4, nsamp // 8)]
-        refh = orc.me_batch(cfg["proc"], ev[hard])
+    bound = parity_bound(ev[idx], cfg["sqrt_s"]) if name.startswith("ggttg") else np.full(nfirst, TOL64)
+    rec = report("%s first %d" % (name, nfirst), rel, bound)
+    assert rec["above_bound"] == 0 and rec["median"] < 1e-12, rec
+    if nhard:
+        hard = np.argsort(min_gluon_invariant(ev))[:nhard]
+        refh = oracle_ld.me_batch(cfg["proc"], ev[hard])
         relh = np.abs(me[hard] / refh - 1)
-        assert relh.max() < 1e-8 and np.median(relh) < 1e-9, (relh.max(), np.median(relh))
+        rech = report("%s hardest %d of %d" % (name, nhard, nevt), relh, parity_bound(ev[hard], cfg["sqrt_s"]))
+        assert rech["above_bound"] == 0, rech
+    # a random sample across the whole batch (tiles, tails)
+    rng = np.random.default_rng(12345)
+    samp = rng.choice(nevt, size=min(nevt, {"ggttggg": 24}.get(name, 512)), replace=False)
+    samp[:2] = [nevt - 1, nevt // 2]
+    refs = oracle_ld.me_batch(cfg["proc"], ev[samp])
+    rels = np.abs(me[samp] / refs - 1)
+    assert np.all(rels <= (parity_bound(ev[samp], cfg["sqrt_s"]) if name.startswith("ggttg") else TOL64)), rels.max()
 
 
 def test_golden_worked_examples(mg):
@@ -189,14 +229,15 @@ def test_closed_forms_on_gpu(mg):
 # ------------------------------------------------------------------------------------------ helicities
 def test_helicity_filter_counts_and_per_helicity(mg, oracle):
     import torch
-    want = {"eemumu": (4, 4), "ggtt": (12, 6), "ggttg": (32, 16), "ggttgg": (64, 32), "ggttggg": (128, 64)}
+    want = {"eemumu": (4, 3), "ggtt": (12, 6), "ggttg": (32, 16), "ggttgg": (64, 32), "ggttggg": (128, 64)}
     for name, (ngood, neval) in want.items():
         cfg = workloads.CONFIGS[name]
         proc = mg.Process(cfg["proc"])
         mom, ev = gpu_events(mg, proc, cfg, 4096)
         good = proc.helicity_probe(mom, 4096)
         assert len(good) == ngood == proc.info.ngoodhel
-        # helicity-flip symmetry: QCD helicities pair up (evaluated once, counted twice); e+e- (Z exchange) does not
+        # helicity-flip symmetry: QCD helicities pair up (evaluated once, counted twice); with Z exchange only the pair
+        # e-L e+R -> mu-R mu+L / e-R e+L -> mu-L mu+R (coupling gL gR in both) has equal |M_h|^2
         assert proc.info.nhel_evaluated == neval
         # per-helicity |M_h|^2 is basis independent in a fixed frame (reading A8): compare to the oracle
         ph = proc.sigma_per_helicity(mom, 64).cpu().numpy()
@@ -291,3 +332,65 @@ def test_caller_workspace_and_event_tiles_give_identical_results(mg, name, nevt,
         proc.set_workspace(tiny)
     proc.set_workspace(None)
     assert np.array_equal(proc.sigma(mom, nevt).cpu().numpy(), ref)
+
+
+# ------------------------------------------------------------------------------------------ batch-unweighting primitive
+@pytest.mark.parametrize("precision", ["fp64", "fp32"])
+def test_weight_max_matches_oracle(mg, oracle_ld, precision):
+    """mg_weight_max (PAPER.md:99-:103): products bit-exact, maximum bit-exact, sums to rounding, bit-reproducible."""
+    import torch
+    cfg = workloads.CONFIGS["ggttg"]
+    prec = mg.FP64 if precision == "fp64" else mg.FP32
+    proc = mg.Process(cfg["proc"], precision=prec)
+    for nevt in (0, 1, 255, 8193, 300001):
+        mom, w = proc.rambo(cfg["seed"], cfg["sqrt_s"], max(nevt, 1), weights=True)
+        me = proc.sigma(mom, max(nevt, 1))[:nevt].clone()
+        w = (w[:nevt] * 1e-6).clone()
+        me0 = me.cpu().numpy().astype(np.float64)
+        prod_ref, out_ref = oracle_ld.weight_max(me0, w.cpu().numpy(), single=(precision == "fp32"))
+        out = proc.weight_max(me, w, nevt)
+        got = out.cpu().numpy()
+        assert np.array_equal(me.cpu().numpy().astype(np.float64), prod_ref)         # in-place products, one rounding
+        assert got[0] == out_ref[0]                                                   # the maximum is exact
+        if nevt:
+            assert abs(got[1] / out_ref[1] - 1) < 1e-13 and abs(got[2] / out_ref[2] - 1) < 1e-13
+        else:
+            assert got[0] == -math.inf and got[1] == 0 and got[2] == 0
+        # fixed reduction tree: bit-reproducible
+        me2 = torch.from_numpy(me0).to(me.dtype).cuda()
+        assert torch.equal(proc.weight_max(me2, w, nevt), out)
+
+
+def test_helicity_all_mode_ignores_the_probe(mg):
+    cfg = workloads.CONFIGS["ggtt"]
+    proc = mg.Process(cfg["proc"], helicity_mode=mg.HEL_ALL)
+    mom = proc.rambo(cfg["seed"], cfg["sqrt_s"], 512)
+    assert len(proc.helicity_probe(mom, 512)) == 16 and proc.info.nhel_evaluated == 16
+    ref = mg.Process(cfg["proc"])
+    a, b = proc.sigma(mom, 512).cpu().numpy(), ref.sigma(mom, 512).cpu().numpy()
+    assert ref.info.nhel_evaluated == 6 and np.max(np.abs(a / b - 1)) < 1e-13
+
+
+def test_bad_derived_couplings_are_rejected(mg):
+    import ctypes as C
+    L = mg.lib()
+    h = C.c_void_p()
+    for kw in (dict(gf=0.0), dict(gf=1e-9), dict(gamma_z=-1.0), dict(sw2=1.5)):
+        p = mg.default_params(**kw)
+        assert L.mg_process_create(b"e+ e- > mu+ mu-", C.byref(p), C.byref(h)) == -3, kw
+
+
+def test_handles_on_two_devices(mg):
+    """A handle created on a second device launches its kernels there (per-device kernel attributes)."""
+    import torch
+    if torch.cuda.device_count() < 2:
+        pytest.skip("needs two visible GPUs")
+    cfg = workloads.CONFIGS["ggttgg"]
+    p0 = mg.Process(cfg["proc"], device=0)
+    p1 = mg.Process(cfg["proc"], device=1)
+    m0 = p0.rambo(cfg["seed"], cfg["sqrt_s"], 1000)
+    with torch.cuda.device(1):
+        m1 = p1.rambo(cfg["seed"], cfg["sqrt_s"], 1000)
+        b = p1.sigma(m1, 1000).cpu().numpy()
+    a = p0.sigma(m0, 1000).cpu().numpy()
+    assert np.array_equal(a, b)

@@ -110,7 +110,7 @@ def test_worked_examples(oracle_ld):
 
 
 # ---------------------------------------------------------------- independent second route
-@pytest.mark.parametrize("nfinal,nev", [(0, 5), (1, 5), (2, 1)])
+@pytest.mark.parametrize("nfinal,nev", [(0, 5), (1, 5), (2, 3)])
 def test_colour_ordered_equals_colour_dressed(oracle, nfinal, nev):
     masses = [173.0, 173.0] + [0.0] * nfinal
     mom = oracle.rambo(100 + nfinal, nev, masses, 1500.0)
