@@ -63,12 +63,12 @@ static void free_all(mg_process* p) {
   cudaGetLastError();
 }
 
-// Workspace of the event-CTA shape: JAMP scratch for every resident CTA (at most 4 per SM) + the per-event invariants
+// Workspace of the event-CTA shape: JAMP scratch for every resident CTA (desc->ctas_per_sm per SM) + the per-event invariants
 // of one event tile.  Library-owned by default: sized for the whole batch, capped at MG_WS_DEFAULT_CAP, grown on
 // demand (synchronously), never shrunk; or caller-provided through mg_set_workspace.
 static const size_t MG_WS_DEFAULT_CAP = (size_t)1 << 30;
 static size_t ws_scratch_bytes(const mg_process* p) {
-  return (size_t)4 * p->nsm * (size_t)p->desc->ws_bytes_per_cta[p->par.precision == MG_FP64 ? 0 : 1];
+  return (size_t)p->desc->ctas_per_sm * p->nsm * (size_t)p->desc->ws_bytes_per_cta[p->par.precision == MG_FP64 ? 0 : 1];
 }
 static size_t ws_need(const mg_process* p, int64_t nevt) {
   const size_t per_e = (size_t)p->desc->ws_bytes_per_event[p->par.precision == MG_FP64 ? 0 : 1];

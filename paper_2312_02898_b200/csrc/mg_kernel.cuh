@@ -63,6 +63,7 @@ struct mg_procdesc_t {
   long long flops_algorithmic_per_event;   // same with every table built once per slot
   int ws_bytes_per_cta[2];   // JAMP scratch per resident CTA for fp64 / fp32
   int nlane;                 // event-CTA shape: helicity lanes per slot = 2^(npar-1)
+  int ctas_per_sm;           // event-CTA shape: resident CTAs per SM the launcher uses at most (sizes the JAMP scratch)
 };
 // both launch functions return the number of kernels they launched (< 0: error).
 #endif  // __CUDACC__

@@ -556,15 +556,15 @@ def _main_unit(E, n, ns, hdr, cfi, cfden, fams, bodies, bmeta, invmap, flowmap, 
                             "    T meh = s_meh[tid];" if dmma else
                             "T meh = colour_reg<T>(jamp);"),
                     coloursm=(2 * ncol * 34 + (BLK // 32) * 32) * 8 if dmma else 0))
-    w(LAUNCH % dict(cfden=cfden, denom=denom,
+    w(LAUNCH % dict(cfden=cfden, denom=denom, minb=cfg.get("ctas_per_sm", 256 // BLK),
                     run32=("  return run<float>(mom, (float*)me_out, nevt, (const float*)lane_w, ntb, tb_first, (float*)perhel_out, par, ws, ws_bytes, st);"
                            if fp32 else "  return -1;")))
     w("}  // namespace\n")
     w("extern const mg_procdesc_t mg_desc_%s = {\"%s\", %d, %d, %d, %d, %d, %d,\n"
-      "  %dLL, {0, 0, 1, 1%s}, nullptr, %s::launch, {0, 0}, 2, %d, {%d, %d}, %dLL, %dLL, %dLL, {%d, %d}, %d};\n"
+      "  %dLL, {0, 0, 1, 1%s}, nullptr, %s::launch, {0, 0}, 2, %d, {%d, %d}, %dLL, %dLL, %dLL, {%d, %d}, %d, %d};\n"
       % (ns[3:], hdr["proc"], npar, n, hdr["ndiag"], nhel, ncol, denom, flops_hel, ", 0" * (n - 2), ns, 1 if fp32 else 0,
          ninvp * 8, ninvp * 4, algo_hel, flops_slot, algo_slot, (2 * ncol * BLK + (BLK // hdr["nlane"]) * ntabf) * 8,
-         (2 * ncol * BLK + (BLK // hdr["nlane"]) * ntabf) * 4, hdr["nlane"]))
+         (2 * ncol * BLK + (BLK // hdr["nlane"]) * ntabf) * 4, hdr["nlane"], cfg.get("ctas_per_sm", 256 // BLK)))
     return (ns + ".cu", "".join(out))
 
 
@@ -660,7 +660,7 @@ static int run(const double* mom, T* me_out, long long nevt, const T* lane_w, in
   auto kern = sigma_kernel<T>;
   if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return -1;
   if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, BLK, smem) != cudaSuccess || per_sm < 1) return -1;
-  if (per_sm > 4) per_sm = 4;                             // mg_api.cu sizes the scratch for at most 4 CTAs per SM
+  if (per_sm > %(minb)d) per_sm = %(minb)d;                             // mg_api.cu sizes the scratch for this many CTAs per SM
   const long long ncta_max = (long long)per_sm * nsm;
   const size_t per_cta = (size_t)2 * NCOL * BLK + (size_t)SLOTS * NTABF;
   const size_t scratch_bytes = (size_t)ncta_max * per_cta * sizeof(T);
