@@ -113,6 +113,26 @@ def dram_traffic(name, precision):
     return None
 
 
+def measured_flops(name, precision):
+    """FP64 FLOPs per event of one mg_sigma call as counted by ncu (dadd + dmul + 2 dfma + 512 per DMMA), and the
+    generator's static counts, from profiles/r2_flops.csv (columns: workload, precision, measured_flops_per_event,
+    static_executed_per_event, static_algorithmic_per_event, source); None if absent."""
+    path = os.path.join(ROOT, "profiles", "r2_flops.csv")
+    if not os.path.exists(path):
+        return None
+    for line in open(path):
+        f = [x.strip() for x in line.split(",")]
+        if len(f) >= 6 and f[0] == name and f[1] == precision:
+            return dict(measured=float(f[2]), static_executed=float(f[3]), static_algorithmic=float(f[4]), source=f[5])
+    return None
+
+
+# per-event FLOPs of round 1's kernels (its generator's static algorithmic count, BENCH_r01.json / DESIGN.md §7):
+# the same |M|^2 costs fewer FLOPs now (helicity-flip symmetry, helicity tables); "frac_r1_flop_model" rates today's
+# ME/s with round 1's FLOPs per ME so that the two rounds' roofline fractions can be compared like for like
+R1_FLOPS_PER_EVENT = {("ggttgg", "fp64"): 1760640.0, ("ggttggg", "fp64"): 33470976.0}
+
+
 def measured_peaks(device):
     """DFMA / FFMA / DMMA rates of the device measured now with the helper library libmg5b200_peak.so (FLOP/s)."""
     import ctypes as C
@@ -246,6 +266,10 @@ def measure(mg, torch, dist, name, cfg, args, steps, rank, world, local, peaks, 
     launches_per_step = int(info.launches_last_sigma) + 1            # the sigma kernels + the RAMBO kernel
     flops_call = float(info.flops_per_event_goodhel) * nevt          # generator's static (algorithmic) count, FMA = 2
     executed = float(info.flops_executed_per_event_goodhel) * nevt   # including diagram-group recomputation
+    mf = None if args.nevt else measured_flops(name, args.precision)
+    stale = mf is not None and abs(mf["static_algorithmic"] / float(info.flops_per_event_goodhel) - 1) > 0.02
+    if mf is not None and not stale:                                  # ncu counters of this kernel set: the numerator
+        flops_call = min(flops_call, mf["measured"] * nevt)
     achieved = flops_call * steps / t_sigma
     fp64 = prec == mg.FP64
     peak_meas = peaks["dfma" if fp64 else "ffma"]
@@ -276,7 +300,13 @@ def measure(mg, torch, dist, name, cfg, args, steps, rank, world, local, peaks, 
                      "algorithmic_bytes": nevt * (32 * info.npar + me.element_size()),
                      "kernel": "mg_sigma: all kernels of one call, timed together with CUDA events (%d launches)"
                                % int(info.launches_last_sigma),
-                     "flops_per_event": int(info.flops_per_event_goodhel), "ngoodhel": int(info.ngoodhel),
+                     "flops_per_event": flops_call / nevt, "flops_per_event_static_algorithmic": int(info.flops_per_event_goodhel),
+                     "flops_per_event_ncu": None if mf is None else mf["measured"],
+                     "flops_source": ("generator's static algorithmic count (mg_process_info)" if mf is None or stale else
+                                      "min(static algorithmic count, ncu dadd+dmul+2*dfma+512*dmma per event from %s)" % mf["source"]),
+                     "frac_r1_flop_model": (None if (name, args.precision) not in R1_FLOPS_PER_EVENT else
+                                            R1_FLOPS_PER_EVENT[(name, args.precision)] * nevt * steps / t_sigma / peak),
+                     "ngoodhel": int(info.ngoodhel),
                      "nhel_evaluated": int(info.nhel_evaluated),
                      "executed_tflops": executed * steps / t_sigma / 1e12,
                      "executed_frac": executed * steps / t_sigma / peak,

@@ -32,7 +32,9 @@ from .tables import Tables, KIND, gluon_particle
 BLK = 256      # default threads per CTA (cfg["block"])
 # body sizes, table thresholds (gluon currents over <= gtab leaves and quark-line currents with <= qtab absorbed gluons
 # come from the per-visit helicity tables) and the shared-memory budget, per multiplicity
-TUNED = {4: dict(max_phase=24, gtab=3, qtab=2, smem_kb=110, block=128, sync_every=0),
+# (measured on B200: gg -> tt~gg 37.9 ms with (2, 1) tables and 40-term bodies against 40.6 ms with (3, 2)
+# and 24; gg -> tt~ggg 424 ms with (3, 2) and 16-term bodies against 500 / 562 ms with 32 / 48)
+TUNED = {4: dict(max_phase=40, gtab=2, qtab=1, smem_kb=110, block=128, sync_every=0),
          5: dict(max_phase=16, gtab=3, qtab=2, smem_kb=110, block=128, sync_every=0)}
 INV_SIZE = {"sg": 1, "pm": 4, "tl": 5, "tr": 5, "eg": 5, "ub": 16, "vv": 16}
 _ORDER = {"s": 0, "p": 1, "t": 2, "e": 3, "u": 4, "v": 5}
@@ -64,48 +66,58 @@ def _perm_name(name, pi):
     return name          # ub, vv
 
 
-def families(n, max_phase):
+def _pack(groups, limit):
+    """First-fit-decreasing packing of term groups (kept whole when they fit) into bodies of <= limit terms."""
+    bodies = []
+    for g in sorted(groups, key=lambda g: -len(g)):
+        while len(g) > limit:
+            bodies.append(g[:limit])
+            g = g[limit:]
+        for b in bodies:
+            if len(b) + len(g) <= limit:
+                b.extend(g)
+                break
+        else:
+            bodies.append(list(g))
+    return [b for b in bodies if b]
+
+
+def families(n, max_phase, min_class=6):
     """[dict(kind, size, members=[pi, ...], bodies=[[term, ...], ...])]: the canonical class of every family, cut into
-    bodies, and the relabellings pi (tuples: canonical gluon i -> actual gluon pi[i]) of its members."""
+    bodies, and the relabellings pi (tuples: canonical gluon i -> actual gluon pi[i]) of its members.  Classes with
+    fewer than `min_class` terms are not worth a visit per member: their terms are emitted as they are, together, in a
+    last family with the identity as its only member."""
     classes = {}
     for term in topo.diagram_terms(n):
         kind, S = family_key(term, n)
         classes.setdefault((kind, len(S)), {}).setdefault(S, []).append(term)
-    out = []
+    out, misc = [], []
     for (kind, size), cls in sorted(classes.items()):
         sizes = {len(v) for v in cls.values()}
-        if len(sizes) == 1 and len(cls) == comb(n, size):
-            S0 = min(cls)
-            rest0 = [i for i in range(n) if i not in S0]
-            members = []
-            for S in sorted(cls):
-                rest = [i for i in range(n) if i not in S]
-                pi = [0] * n
-                for a, b in zip(S0, S):
-                    pi[a] = b
-                for a, b in zip(rest0, rest):
-                    pi[a] = b
-                members.append(tuple(pi))
-            terms0 = cls[S0]
-        else:               # the key of this kind is not equivariant (ties): one member, every term
-            members = [tuple(range(n))]
-            terms0 = [t for S in sorted(cls) for t in cls[S]]
+        if not (len(sizes) == 1 and len(cls) == comb(n, size)) or min(sizes) < min_class:
+            misc += [t for S in sorted(cls) for t in cls[S]]      # key not equivariant (ties), or class too small
+            continue
+        S0 = min(cls)
+        rest0 = [i for i in range(n) if i not in S0]
+        members = []
+        for S in sorted(cls):
+            rest = [i for i in range(n) if i not in S]
+            pi = [0] * n
+            for a, b in zip(S0, S):
+                pi[a] = b
+            for a, b in zip(rest0, rest):
+                pi[a] = b
+            members.append(tuple(pi))
         # bodies: terms that share their fine key (the big sub-tree they hang on) stay together
         fine = {}
-        for t in terms0:
+        for t in cls[S0]:
             fine.setdefault(repr(group_key(t, n)[1]), []).append(t)
-        bodies, cur = [], []
-        for fk in sorted(fine):
-            if cur and len(cur) + len(fine[fk]) > max_phase:
-                bodies.append(cur)
-                cur = []
-            cur = cur + fine[fk]
-            while len(cur) > max_phase:
-                bodies.append(cur[:max_phase])
-                cur = cur[max_phase:]
-        if cur:
-            bodies.append(cur)
-        out.append(dict(kind=kind, size=size, members=members, bodies=bodies))
+        out.append(dict(kind=kind, size=size, members=members, bodies=_pack([fine[k] for k in sorted(fine)], max_phase)))
+    if misc:
+        fine = {}
+        for t in misc:
+            fine.setdefault(repr(group_key(t, n)), []).append(t)
+        out.append(dict(kind="X", size=0, members=[tuple(range(n))], bodies=_pack([fine[k] for k in sorted(fine)], max_phase)))
     return out
 
 
@@ -279,7 +291,7 @@ def emit_coop(n, fp32=True, acc_max=24, **over):
     cfi = [[int(v * cfden) for v in row] for row in cf]
     flow_index = topo.flow_index_table(n)
     flow_order = {i: p for p, i in flow_index.items()}
-    fams = families(n, cfg["max_phase"])
+    fams = families(n, cfg["max_phase"], cfg.get("min_class", 6))
     # bodies are compiled for the register budget of the kernel's occupancy target (build.py reads the "nvcc:" line)
     maxreg = min(255, 65536 // (BLK * cfg.get("ctas_per_sm", 256 // BLK)) // 8 * 8)
     hdr = dict(proc=proc, n=n, ncol=ncol, nhel=nhel, ns=ns, npar=npar, nlane=nlane, blk=BLK,
@@ -320,7 +332,8 @@ def emit_coop(n, fp32=True, acc_max=24, **over):
     for bi, (fi, b) in enumerate(bodies):
         fam = fams[fi]
         nm_ = len(fam["members"])
-        flops = b.plan.flops_per_helicity(colour=False, externals=False)
+        # executed: the relabelling sign costs one complex scaling (2 multiplications) per amplitude
+        flops = b.plan.flops_per_helicity(colour=False, externals=False) + 2 * b.plan.namps
         exec_hel += flops * nm_
         touches = {}
         for op in b.plan.ops:

@@ -34,11 +34,15 @@ from math import factorial
 
 from . import topology as topo
 
-# static FLOP counts per routine (DFMA = 2, DMUL/DADD = 1), counted from mg_wave.cuh by hand; used only
-# for mg_process_info()'s algorithmic FLOP figure — measured FLOPs come from ncu.
-FLOPS = {"v3": 4 * 7 + 2 * 7 * 2 + 12 + 6 + 4 * (1 + 9 * 2 + 1), "k": 3 * 4 * 7 + 8 + 4 * 2 * 11,
-         "lq": 8 + 2 * 28 + 8 + 8 * 9, "rq": 8 + 2 * 28 + 8 + 8 * 9, "bil": 16 * 3 + 24, "amp": 4 * 7,
-         "ext_g": 30, "ext_q": 50, "jamp_add": 2}
+# static FLOP counts per routine (DFMA = 2, DMUL/DADD = 1), counted from the expressions in mg_wave.cuh as ptxas
+# contracts them (a complex product component = 1 mul + 1 fma; a 4-term dot product component = 1 mul + 7 fma, ...):
+#   v3  wdot 30 + 2 pwdot 28 + (2 PB + PA, 2 PA + PB) 16 + scalings 6 + 4 components x (1 + 9 + 9) = 156
+#   k   3 wdot 45 + scalings 8 + 4 components x (11 + 11) = 141
+#   lq/rq  slash blocks 8 + two 2x2 complex row/column products 56 + 8 components x (1 mul + 3 fma) = 120
+#   bil 16 real products-of-complex (3 each) + 24 adds = 72;  amp 2 x (1 mul + 7 fma) = 30
+# Cross-checked against ncu's dadd/dmul/dfma thread-instruction counters for whole mg_sigma calls
+# (profiles/r2_flops.md: static / measured = 1.00-1.03); mg_process_info() reports the static figures.
+FLOPS = {"v3": 156, "k": 141, "lq": 120, "rq": 120, "bil": 72, "amp": 30, "ext_g": 30, "ext_q": 50, "jamp_add": 2}
 
 
 def closure_block(term):
