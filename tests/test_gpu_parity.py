@@ -380,6 +380,21 @@ def test_weight_max_matches_oracle(mg, oracle_ld, precision):
         assert torch.equal(proc.weight_max(me2, w, nevt), out)
 
 
+@pytest.mark.parametrize("name,nevt", [("ggttgg", 30011), ("ggttggg", 4001)])
+def test_results_are_bit_reproducible(mg, name, nevt):
+    """The JAMP accumulation (L2 reductions into thread-private addresses, issued in program order), the colour sum and
+    the helicity sum (fixed trees) have a fixed order: repeated calls, and calls on another handle, agree bit for bit.
+    (compute-sanitizer is not available on this GPU pool; a race in the shared-memory visit pipeline or in the JAMP
+    scratch would show up here and in the bit-exact tiling test above.)"""
+    cfg = workloads.CONFIGS[name]
+    p1, p2 = mg.Process(cfg["proc"]), mg.Process(cfg["proc"])
+    mom = p1.rambo(cfg["seed"], cfg["sqrt_s"], nevt)
+    a = p1.sigma(mom, nevt).cpu().numpy()
+    for _ in range(3):
+        assert np.array_equal(p1.sigma(mom, nevt).cpu().numpy(), a)
+    assert np.array_equal(p2.sigma(mom, nevt).cpu().numpy(), a)
+
+
 def test_helicity_all_mode_ignores_the_probe(mg):
     cfg = workloads.CONFIGS["ggtt"]
     proc = mg.Process(cfg["proc"], helicity_mode=mg.HEL_ALL)
