@@ -144,6 +144,20 @@ int mg_helicity_probe(mg_process_t* p, const void* momenta_dev, int64_t nprobe, 
 int mg_sigma_per_helicity(mg_process_t* p, const void* momenta_dev, int64_t nevt, void* perhel_out_dev,
                           void* stream);
 /* Copies the current good-helicity list (indices; bit (npar-1-i) set <=> particle i has lambda=+1). */
+/* Mixed precision with precision tracking ("tracking the precision of the matrix elements
+ * showed that single-precision computations are not accurate enough"): on an MG_FP64 handle of a process that has fp32
+ * kernels (all but g g > t t~ g g g), evaluates every helicity in fp32, measures per event
+ *     eps = sum over mirror pairs | |M_h|^2 - |M_hbar|^2 | / sum_h |M_h|^2  +  2^-26 s / (2 min_ij |p_i.p_j|)
+ * (hbar = all helicities flipped: the first term is zero in exact arithmetic, i.e. it measures the event's fp32
+ * arithmetic error; the second, over pairs of massless legs of the gluon processes, covers the rounding of the inputs
+ * the two mirrors share, which grows with the event's conditioning), and re-evaluates in fp64 the events with
+ * eps > tol (or a non-finite value).  me_out_dev: nevt doubles (fp32 sums for the
+ * events kept, fp64 values for the re-evaluated ones); eps_out_dev: NULL or nevt floats; *nflagged_out (host, may be
+ * NULL): number of re-evaluated events.  Synchronises the stream once (the count).  MG_ERR_BAD_PARAM on an MG_FP32
+ * handle, a process without fp32 kernels, or tol < 0. */
+int mg_sigma_mixed(mg_process_t* p, const void* momenta_dev, int64_t nevt, double* me_out_dev, double tol,
+                   float* eps_out_dev, int64_t* nflagged_out, void* stream);
+
 int mg_good_helicities(const mg_process_t* p, int32_t* out, int32_t capacity, int32_t* ngood);
 
 int mg_process_info(const mg_process_t* p, mg_info_t* out);

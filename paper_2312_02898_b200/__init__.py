@@ -20,7 +20,7 @@ HEL_FILTER, HEL_ALL = 0, 1
 
 SYMBOLS = ["mg_params_default", "mg_process_create", "mg_process_destroy", "mg_rambo", "mg_rambo_ex", "mg_philox_raw", "mg_sigma",
            "mg_sigma_host", "mg_helicity_probe", "mg_sigma_per_helicity", "mg_good_helicities", "mg_process_info",
-           "mg_momenta_bytes", "mg_set_workspace", "mg_workspace_bytes", "mg_weight_max", "mg_status_string", "mg_last_error"]
+           "mg_momenta_bytes", "mg_set_workspace", "mg_workspace_bytes", "mg_weight_max", "mg_sigma_mixed", "mg_status_string", "mg_last_error"]
 
 
 class MgParams(C.Structure):
@@ -74,6 +74,7 @@ def lib():
         L.mg_workspace_bytes.argtypes = [vp, i64]
         L.mg_workspace_bytes.restype = C.c_size_t
         L.mg_weight_max.argtypes = [vp, vp, vp, i64, vp, vp]
+        L.mg_sigma_mixed.argtypes = [vp, vp, i64, vp, C.c_double, vp, C.POINTER(i64), vp]
         L.mg_status_string.argtypes = [C.c_int]
         L.mg_status_string.restype = C.c_char_p
         L.mg_last_error.restype = C.c_char_p
@@ -212,6 +213,17 @@ class Process:
         _check(lib().mg_weight_max(self._h, C.c_void_p(me.data_ptr()), C.c_void_p(weights.data_ptr()), nevt,
                                    C.c_void_p(res.data_ptr()), _stream_ptr(stream)))
         return res
+
+    def sigma_mixed(self, momenta, nevt, tol, with_eps=False, stream=None):
+        """mg_sigma_mixed: fp32 everywhere, fp64 where the measured fp32 error exceeds tol.  Returns (|M|^2 as a
+        float64 device tensor, number of re-evaluated events[, eps as a float32 device tensor])."""
+        import torch
+        me = torch.empty(nevt, dtype=torch.float64, device=momenta.device)
+        eps = torch.empty(nevt, dtype=torch.float32, device=momenta.device) if with_eps else None
+        nf = C.c_int64()
+        _check(lib().mg_sigma_mixed(self._h, C.c_void_p(momenta.data_ptr()), nevt, C.c_void_p(me.data_ptr()), float(tol),
+                                    C.c_void_p(eps.data_ptr()) if with_eps else None, C.byref(nf), _stream_ptr(stream)))
+        return (me, nf.value, eps) if with_eps else (me, nf.value)
 
     def good_helicities(self):
         n = C.c_int32()

@@ -50,6 +50,8 @@ struct mg_process {
   void* io_mom = nullptr; size_t io_mom_bytes = 0;   // device staging of mg_sigma_host (grow-only, library-owned)
   void* io_out = nullptr; size_t io_out_bytes = 0;
   void* ws = nullptr; size_t ws_bytes = 0; bool ws_user = false;   // event-CTA shape: JAMP scratch + per-event invariants
+  void* lanew_all32_dev = nullptr;   // ones as float: fp32 pass of mg_sigma_mixed on an fp64 handle
+  void* mx = nullptr; size_t mx_bytes = 0;   // scratch of mg_sigma_mixed (grow-only, library-owned)
 };
 
 static size_t esize(const mg_process_t* p) { return p->par.precision == MG_FP64 ? 8 : 4; }
@@ -58,6 +60,7 @@ static void free_all(mg_process* p) {
   cudaFree(p->hel_dev); cudaFree(p->hel_all_dev); cudaFree(p->helw_dev); cudaFree(p->ones_dev);
   cudaFree(p->lanew_dev); cudaFree(p->lanew_all_dev); cudaFree(p->stats_dev); cudaFree(p->wpart_dev);
   if (p->ws && !p->ws_user) cudaFree(p->ws);
+  cudaFree(p->lanew_all32_dev); cudaFree(p->mx);
   if (p->io_mom) cudaFree(p->io_mom);
   if (p->io_out) cudaFree(p->io_out);
   cudaGetLastError();
@@ -221,6 +224,8 @@ int mg_process_create(const char* proc, const mg_params_t* params, mg_process_t*
     if (ce == cudaSuccess) ce = cudaMalloc(&p->lanew_all_dev, es * 2 * d->nlane);
     if (ce == cudaSuccess) ce = cudaMemcpy(p->lanew_all_dev, es == 8 ? (const void*)ones.data() : (const void*)onesf.data(),
                                            es * 2 * d->nlane, cudaMemcpyHostToDevice);
+    if (ce == cudaSuccess && d->has_fp32) ce = cudaMalloc(&p->lanew_all32_dev, 4 * 2 * d->nlane);
+    if (ce == cudaSuccess && d->has_fp32) ce = cudaMemcpy(p->lanew_all32_dev, onesf.data(), 4 * 2 * d->nlane, cudaMemcpyHostToDevice);
   }
   if (ce != cudaSuccess) { free_all(p); delete p; return cuda_fail(ce, "mg_process_create: device set-up"); }
   { const int rc = upload_helicities(p); if (rc != MG_OK) { free_all(p); delete p; return rc; } }
@@ -388,6 +393,68 @@ int mg_sigma_host(mg_process_t* p, const void* momenta_host, int64_t nevt, void*
   if (rc != MG_OK) return rc;
   if (e != cudaSuccess) return cuda_fail(e, "mg_sigma_host copy");
   if (es != cudaSuccess) return cuda_fail(es, "mg_sigma_host sync");
+  return MG_OK;
+}
+
+int mg_sigma_mixed(mg_process_t* p, const void* momenta_dev, int64_t nevt, double* me_out_dev, double tol,
+                   float* eps_out_dev, int64_t* nflagged_out, void* stream) {
+  if (!p || ((!momenta_dev || !me_out_dev) && nevt > 0)) return MG_ERR_NULL;
+  if (nevt < 0 || nevt > 0x7fffffff) return MG_ERR_BAD_NEVT;
+  if (((uintptr_t)momenta_dev & 15) || ((uintptr_t)me_out_dev & 7) || ((uintptr_t)eps_out_dev & 3)) return MG_ERR_ALIGN;
+  if (p->par.precision != MG_FP64 || !p->desc->has_fp32 || !(tol >= 0)) return MG_ERR_BAD_PARAM;
+  if (nflagged_out) *nflagged_out = 0;
+  if (nevt == 0) return MG_OK;
+  const mg_procdesc_t* d = p->desc;
+  cudaStream_t st = (cudaStream_t)stream;
+  MG_CUDA(cudaSetDevice(p->par.device));
+  if (!p->probed) {                        // the fp64 re-evaluation uses the handle's helicity state
+    const int rc = mg_helicity_probe(p, momenta_dev, nevt < 4096 ? nevt : 4096, stream);
+    if (rc != MG_OK) return rc;
+  }
+  // scratch: perhel32 [nhel][nevt] | me32 [nevt] | flagged [nevt] + counter | compact momenta | compact |M|^2
+  const size_t npad = (size_t)(nevt + 31) / 32 * 32;
+  const size_t o_me32 = (size_t)d->nhel * nevt * 4, o_flag = o_me32 + npad * 4, o_cnt = o_flag + npad * 4;
+  const size_t o_mom = (o_cnt + 256) / 256 * 256, o_me64 = o_mom + npad * d->npar * 32, need = o_me64 + npad * 8;
+  if (p->mx_bytes < need) {
+    if (p->mx) { cudaDeviceSynchronize(); cudaFree(p->mx); p->mx = nullptr; p->mx_bytes = 0; }
+    MG_CUDA(cudaMalloc(&p->mx, need));
+    p->mx_bytes = need;
+  }
+  char* base = (char*)p->mx;
+  float* perhel = (float*)base;
+  int* flagged = (int*)(base + o_flag);
+  int* cnt = (int*)(base + o_cnt);
+  // 1. fp32 pass, every helicity, per-helicity output
+  long long n;
+  if (d->launch) n = d->launch(MG_FP32, (const double*)momenta_dev, base + o_me32, nevt, p->hel_all_dev, p->ones_dev, d->nhel, perhel, p->pvec, st);
+  else {
+    { const int rc = ensure_ws(p, nevt); if (rc != MG_OK) return rc; }
+    n = d->launch_slots(MG_FP32, (const double*)momenta_dev, base + o_me32, nevt, p->lanew_all32_dev, 2, 0, perhel, p->pvec, p->ws, p->ws_bytes, st);
+  }
+  if (n < 0) { cudaGetLastError(); return fail(MG_ERR_CUDA, "mg_sigma_mixed: fp32 launch set-up failed"); }
+  long long launches = n;
+  // 2. per-event precision estimate, fp32 sums, flags
+  unsigned massless = 0;
+  for (int i = 0; i < d->npar; ++i) if (!d->massive[i]) massless |= 1u << i;
+  const double kappa = d->ngluons > 0 ? 0.25 : 0.0;          // the conditioning term is about soft / collinear gluons
+  MG_CUDA(mg_launch_mixed_flag(perhel, (const double*)momenta_dev, nevt, d->nhel, d->npar, massless, kappa, tol, me_out_dev,
+                               eps_out_dev, flagged, cnt, st));
+  int nf = 0;
+  MG_CUDA(cudaMemcpyAsync(&nf, cnt, sizeof(int), cudaMemcpyDeviceToHost, st));
+  MG_CUDA(cudaStreamSynchronize(st));
+  launches += 1;
+  // 3. fp64 re-evaluation of the flagged events
+  if (nf > 0) {
+    double* cmom = (double*)(base + o_mom);
+    double* cme = (double*)(base + o_me64);
+    MG_CUDA(mg_launch_mixed_gather((const double*)momenta_dev, flagged, nf, d->npar, cmom, st));
+    const int rc = run_sigma(p, cmom, nf, cme, nullptr, false, st);
+    if (rc != MG_OK) return rc;
+    launches += p->launches + 2;
+    MG_CUDA(mg_launch_mixed_scatter(cme, flagged, nf, me_out_dev, st));
+  }
+  p->launches = launches;
+  if (nflagged_out) *nflagged_out = nf;
   return MG_OK;
 }
 

@@ -18,3 +18,9 @@ cudaError_t mg_launch_philox_raw(uint64_t seed, long long first_event, long long
 cudaError_t mg_launch_probe_stats(int prec, const void* perhel, long long nevt, int nhel, double* out, cudaStream_t st);
 int mg_weight_blocks(long long n);
 cudaError_t mg_launch_weight_max(int prec, void* me, const double* w, long long n, double* part, double* out, cudaStream_t st);
+// mixed precision with precision tracking (mg_sigma_mixed)
+cudaError_t mg_launch_mixed_flag(const float* perhel, const double* mom, long long nevt, int nhel, int npar, unsigned massless_mask,
+                                 double kappa, double tol, double* me_out, float* eps_out, int* flagged, int* nflagged,
+                                 cudaStream_t st);
+cudaError_t mg_launch_mixed_gather(const double* mom, const int* flagged, int n, int npar, double* out, cudaStream_t st);
+cudaError_t mg_launch_mixed_scatter(const double* me64, const int* flagged, int n, double* me_out, cudaStream_t st);

@@ -111,3 +111,85 @@ cudaError_t mg_launch_weight_max(int prec, void* me, const double* w, long long 
   weight_stage2<<<1, RB, 0, st>>>(part, nb, out);
   return cudaGetLastError();
 }
+
+// ---- mixed precision with precision tracking ("tracking the precision of the matrix
+// elements showed that single-precision computations are not accurate enough") ----
+// The fp32 kernels evaluate every helicity h and its helicity-flipped mirror hbar; in exact arithmetic |M_h|^2 =
+// |M_hbar|^2 (A13), so  eps = sum_{h < hbar} | |M_h|^2 - |M_hbar|^2 | / sum_h |M_h|^2  is a per-event
+// measurement of the fp32 arithmetic error of that event.  It does not see the rounding of the inputs both mirrors share
+// (the helicity-independent operands are rounded to fp32 once), whose effect grows with the event's conditioning, so the
+// tracker adds  kappa 2^-24 s / (2 min_ij |p_i.p_j|)  over pairs of massless legs (kappa = 1/4, calibrated on the full
+// batches of configs 3-4: DESIGN.md §7).  Events with eps > tol (or a non-finite value) are flagged for re-evaluation
+// in fp64.
+namespace {
+__global__ void __launch_bounds__(RB) mixed_flag_kernel(const float* __restrict__ perhel, const double* __restrict__ mom,
+                                                        long long nevt, int nhel, int npar, unsigned massless_mask, double kappa,
+                                                        double tol, double* __restrict__ me_out, float* __restrict__ eps_out,
+                                                        int* __restrict__ flagged, int* __restrict__ nflagged) {
+  const long long i = (long long)blockIdx.x * RB + threadIdx.x;
+  if (i >= nevt) return;
+  double s = 0.0, a = 0.0;
+  for (int h = 0; h < nhel / 2; ++h) {
+    const double x = (double)perhel[(long long)h * nevt + i], y = (double)perhel[(long long)(nhel - 1 - h) * nevt + i];
+    s += x + y;
+    a += fabs(x - y);
+  }
+  double eps = a / s;
+  if (kappa > 0.0) {
+    const double* pm = mom + ((i / 32) * npar * 32 + (i % 32)) * 4;      // particle ip at pm + ip * 128
+    double dmin = INFINITY;
+    for (int ia = 0; ia < npar; ++ia) {
+      if (!((massless_mask >> ia) & 1)) continue;
+      const double* pa = pm + ia * 128;
+      for (int ib = ia + 1; ib < npar; ++ib) {
+        if (!((massless_mask >> ib) & 1)) continue;
+        const double* pb = pm + ib * 128;
+        const double d = fabs(pa[0] * pb[0] - pa[1] * pb[1] - pa[2] * pb[2] - pa[3] * pb[3]);
+        dmin = d < dmin ? d : dmin;
+      }
+    }
+    const double shat = 2.0 * fabs(pm[0] * pm[128] - pm[1] * pm[129] - pm[2] * pm[130] - pm[3] * pm[131]);   // massless beams
+    eps += kappa * 5.9604644775390625e-08 * shat / (2.0 * dmin);
+  }
+  me_out[i] = s;
+  if (eps_out) eps_out[i] = (float)eps;
+  if (!(eps <= tol) || !(s > 0.0) || isinf(s)) flagged[atomicAdd(nflagged, 1)] = (int)i;
+}
+// flagged events' momenta -> compact AoSoA pages (32 events per page, [page][ipar][32][4])
+__global__ void __launch_bounds__(RB) mixed_gather_kernel(const double* __restrict__ mom, const int* __restrict__ flagged, int n,
+                                                          int npar, double* __restrict__ out) {
+  const int k = blockIdx.x * RB + threadIdx.x;
+  const int npad = (n + 31) / 32 * 32;
+  if (k >= npad) return;
+  const long long i = flagged[k < n ? k : n - 1];            // pad the last page with copies of the last event
+  for (int ip = 0; ip < npar; ++ip) {
+    const double* src = mom + (((i / 32) * npar + ip) * 32 + (i % 32)) * 4;
+    double* dst = out + ((((long long)k / 32) * npar + ip) * 32 + (k % 32)) * 4;
+    dst[0] = src[0]; dst[1] = src[1]; dst[2] = src[2]; dst[3] = src[3];
+  }
+}
+__global__ void __launch_bounds__(RB) mixed_scatter_kernel(const double* __restrict__ me64, const int* __restrict__ flagged, int n,
+                                                           double* __restrict__ me_out) {
+  const int k = blockIdx.x * RB + threadIdx.x;
+  if (k < n) me_out[flagged[k]] = me64[k];
+}
+}  // namespace
+
+cudaError_t mg_launch_mixed_flag(const float* perhel, const double* mom, long long nevt, int nhel, int npar, unsigned massless_mask,
+                                 double kappa, double tol, double* me_out, float* eps_out, int* flagged, int* nflagged,
+                                 cudaStream_t st) {
+  cudaError_t e = cudaMemsetAsync(nflagged, 0, sizeof(int), st);
+  if (e != cudaSuccess) return e;
+  mixed_flag_kernel<<<(unsigned)((nevt + RB - 1) / RB), RB, 0, st>>>(perhel, mom, nevt, nhel, npar, massless_mask, kappa, tol, me_out,
+                                                                    eps_out, flagged, nflagged);
+  return cudaGetLastError();
+}
+cudaError_t mg_launch_mixed_gather(const double* mom, const int* flagged, int n, int npar, double* out, cudaStream_t st) {
+  const int npad = (n + 31) / 32 * 32;
+  mixed_gather_kernel<<<(unsigned)((npad + RB - 1) / RB), RB, 0, st>>>(mom, flagged, n, npar, out);
+  return cudaGetLastError();
+}
+cudaError_t mg_launch_mixed_scatter(const double* me64, const int* flagged, int n, double* me_out, cudaStream_t st) {
+  mixed_scatter_kernel<<<(unsigned)((n + RB - 1) / RB), RB, 0, st>>>(me64, flagged, n, me_out);
+  return cudaGetLastError();
+}

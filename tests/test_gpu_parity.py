@@ -428,3 +428,44 @@ def test_handles_on_two_devices(mg):
         b = p1.sigma(m1, 1000).cpu().numpy()
     a = p0.sigma(m0, 1000).cpu().numpy()
     assert np.array_equal(a, b)
+
+
+# ------------------------------------------------------------------------------------------ mixed precision with tracking
+@pytest.mark.parametrize("name", ["ggttg", "ggttgg"])
+def test_sigma_mixed_tracks_precision(mg, oracle, name):
+    """mg_sigma_mixed: fp32 with a per-event precision estimate, fp64 where it exceeds tol.
+    On the full batch: the estimate flags the events fp32 gets wrong; what is kept is an order of magnitude closer to the
+    fp64 result than plain fp32; tol = 0 re-evaluates everything (= the fp64 path bit for bit); a loose tol none."""
+    import torch
+    cfg = workloads.CONFIGS[name]
+    nevt = cfg["nevt"]
+    proc = mg.Process(cfg["proc"])
+    p32 = mg.Process(cfg["proc"], precision=mg.FP32)
+    mom, ev = gpu_events(mg, proc, cfg, nevt)
+    me64 = proc.sigma(mom, nevt).cpu().numpy()
+    me32 = p32.sigma(mom, nevt).cpu().numpy().astype(np.float64)
+    err32 = np.abs(me32 / me64 - 1)
+    me, nf, eps = proc.sigma_mixed(mom, nevt, 1e-5, with_eps=True)
+    me, eps = me.cpu().numpy(), eps.cpu().numpy()
+    err = np.abs(me / me64 - 1)
+    flagged = ~(eps <= 1e-5)
+    assert nf == int(flagged.sum()) and 0 < nf < 0.05 * nevt
+    assert np.array_equal(me[flagged], me64[flagged])                      # re-evaluated in fp64
+    assert err.max() < 5e-6 < err32.max() and np.median(err) < TOL32_MED
+    print("mixed", name, "plain fp32 max %.2e; mixed (tol 1e-5): %d of %d events in fp64, max %.2e" % (err32.max(), nf, nevt, err.max()))
+    # against the oracle on a sample: the kept fp32 values and the re-evaluated ones
+    idx = np.concatenate([np.arange(256), np.nonzero(flagged)[0][:256]])
+    ref = oracle.me_batch(cfg["proc"], ev[idx])
+    assert np.max(np.abs(me[idx] / ref - 1)) < 5e-6
+    # limits
+    n = 20000
+    me0, nf0 = proc.sigma_mixed(mom, n, 0.0)
+    assert nf0 == n and np.array_equal(me0.cpu().numpy(), me64[:n])
+    me1, nf1 = proc.sigma_mixed(mom, n, 1e9)
+    assert nf1 == 0 and np.max(np.abs(me1.cpu().numpy() / me64[:n] - 1)) < TOL32_MAX
+    # not available: fp32 handle, process without fp32 kernels
+    with pytest.raises(mg.MgError):
+        p32.sigma_mixed(mom, 100, 1e-5)
+    p5 = mg.Process("g g > t t~ g g g")
+    with pytest.raises(mg.MgError):
+        p5.sigma_mixed(p5.rambo(5, 1500.0, 64), 64, 1e-5)
