@@ -430,7 +430,8 @@ def _main_unit(E, n, ns, hdr, cfi, cfden, fams, bodies, bmeta, invmap, flowmap, 
     nbody = len(bodies)
     denom = 4 * 64 * factorial(n - 2)
     rows = E._colour_rows(cfi, ncol)
-    dmma = ncol > 32
+    dmma = ncol > 32 or cfg.get("colour") == "dmma"      # FP64 tensor cores for the colour sum (fp64 kernels only)
+    reg = not dmma or fp32
     out = [HEADER % dict(hdr, nterms=0, flops=flops_hel,
                          what="operand maps, table descriptors, invariants kernel, persistent sigma kernel (%d bodies x their "
                               "relabellings, colour sum K6, helicity sum K7), launcher" % nbody)]
@@ -502,7 +503,7 @@ def _main_unit(E, n, ns, hdr, cfi, cfden, fams, bodies, bmeta, invmap, flowmap, 
         w("};\n")
     w("// symmetric colour form: me = sum_i J_i^* (CF_ii J_i + 2 sum_{j>i} CF_ij J_j) / %d, integer coefficients as immediates\n" % cfden)
     w("template <class T> MG_DEV T colour_reg(const T* __restrict__ jb) {\n")
-    if not dmma:
+    if reg:
         for f in range(ncol):
             w("  const T jr%d = __ldcg(jb + %d * BLK), ji%d = __ldcg(jb + %d * BLK);\n" % (f, 2 * f, f, 2 * f + 1))
         w("  T me = T(0);\n")
@@ -565,8 +566,9 @@ def _main_unit(E, n, ns, hdr, cfi, cfden, fams, bodies, bmeta, invmap, flowmap, 
             "             flow_map + %d + m * %d);\n    }\n"
             % (bi, fams[fi]["kind"], fams[fi]["size"], len(b.plan.terms), nm_, nm_, v0, foff_of[fi], bi, fo, len(b.flows)))
     w(KERNEL % dict(calls="".join(calls), minb=cfg.get("ctas_per_sm", 256 // BLK),
-                    colour=("colour_dmma_cta<NCOL, BLK>(cf_dense, (const double*)jamp_cta, reinterpret_cast<double*>(smem_raw), (double*)s_meh);\n"
-                            "    T meh = s_meh[tid];" if dmma else
+                    colour=("T meh;\n    if constexpr (sizeof(T) == 8) {\n"
+                            "      colour_dmma_cta<NCOL, BLK>(cf_dense, (const double*)jamp_cta, reinterpret_cast<double*>(smem_raw), (double*)s_meh);\n"
+                            "      meh = s_meh[tid];\n    } else meh = colour_reg<T>(jamp);" if dmma else
                             "T meh = colour_reg<T>(jamp);"),
                     coloursm=(2 * ncol * 34 + (BLK // 32) * 32) * 8 if dmma else 0))
     w(LAUNCH % dict(cfden=cfden, denom=denom, minb=cfg.get("ctas_per_sm", 256 // BLK),
