@@ -35,7 +35,7 @@ BLK = 256      # default threads per CTA (cfg["block"])
 # (measured on B200: gg -> tt~gg 37.9 ms with (2, 1) tables and 40-term bodies against 40.6 ms with (3, 2)
 # and 24; gg -> tt~ggg 424 ms with (3, 2) and 16-term bodies against 500 / 562 ms with 32 / 48)
 TUNED = {4: dict(max_phase=40, gtab=2, qtab=1, smem_kb=110, block=128, sync_every=0),
-         5: dict(max_phase=16, gtab=3, qtab=2, smem_kb=110, block=128, sync_every=0)}
+         5: dict(max_phase=16, gtab=3, qtab=2, smem_kb=110, block=128, sync_every=0, min_class=5)}
 INV_SIZE = {"sg": 1, "pm": 4, "tl": 5, "tr": 5, "eg": 5, "ub": 16, "vv": 16}
 _ORDER = {"s": 0, "p": 1, "t": 2, "e": 3, "u": 4, "v": 5}
 
@@ -269,7 +269,7 @@ using namespace mgq;
 constexpr int NPAR = %(npar)d, NGLU = %(n)d, NCOL = %(ncol)d, NHEL = %(nhel)d, NLANE = %(nlane)d, BLK = %(blk)d, SLOTS = BLK / NLANE;
 """
 
-BODY_ARGS = "unsigned sinv, unsigned tab, unsigned sgn, unsigned sj, %s* jamp, int h, int live, const int* fm"
+BODY_ARGS = "unsigned sinv, unsigned tab, unsigned sgn, unsigned sj, %s* jamp, int h, int live, unsigned fm"
 
 
 def emit_coop(n, fp32=True, acc_max=24, **over):
@@ -323,7 +323,10 @@ def emit_coop(n, fp32=True, acc_max=24, **over):
     ntabs = max(b.ntab for _, b in bodies)
     namps = max(b.plan.namps for _, b in bodies)
     assert namps <= BLK
-    fixed = slots * (ninvp + ninvs) * 8 + 2 * namps * 8 + 2 * slots * ntabs * 8 + 3 * ntabs * 4
+    nflows = max(len(b.flows) for _, b in bodies)
+    nflows += nflows & 1
+    assert nflows <= BLK
+    fixed = slots * (ninvp + ninvs) * 8 + 2 * namps * 8 + 2 * slots * ntabs * 8 + 3 * ntabs * 4 + 2 * nflows * 4
     nst_max = max(0, (cfg["smem_kb"] * 1024 - fixed) // (2 * BLK * 8))
     files, binfo = [], []
     exec_hel, exec_slot = 0, 0
@@ -359,8 +362,8 @@ def emit_coop(n, fp32=True, acc_max=24, **over):
                     seen.add(f)
                     w("    ssh(%s, %s%s); ssh(%s, %s%s);\n" % (a, neg, _mul(s, re), b_, neg, _mul(s, im)))
             else:
-                w("    if (live) { T* jp = jamp + __ldg(fm + %d); red_add(jp, %s%s); red_add(jp + BLK, %s%s); }\n"
-                  % (b.slot[f], neg, _mul(s, re), neg, _mul(s, im)))
+                w("    if (live) { T* jp = jamp + ldsi(fm + %du); red_add(jp, %s%s); red_add(jp + BLK, %s%s); }\n"
+                  % (4 * b.slot[f], neg, _mul(s, re), neg, _mul(s, im)))
 
         vaddr = _emit_ops(b, w, sink, sync_every)
         out = [HEADER % dict(hdr, nterms=len(b.plan.terms), flops=flops,
@@ -368,7 +371,7 @@ def emit_coop(n, fp32=True, acc_max=24, **over):
                                   % (bi, nbody, fam["kind"], fam["size"], nm_))]
         o = out.append
         o("template <class T>\nMG_DEV void body%d_impl(const unsigned sinv, const unsigned tab, const unsigned sgn, const unsigned sj,\n"
-          "                      T* __restrict__ jamp, const int h, const int live, const int* __restrict__ fm) {\n" % bi)
+          "                      T* __restrict__ jamp, const int h, const int live, const unsigned fm) {\n" % bi)
         o("  constexpr unsigned SZ = (unsigned)sizeof(T), COL = (unsigned)BLK * SZ;\n")
         for bits, nm in sorted(vaddr.items()):
             if bits:
@@ -380,8 +383,8 @@ def emit_coop(n, fp32=True, acc_max=24, **over):
         if staged:
             o("  if (live) {\n")
             for f, sl in sorted(staged.items()):
-                o("    { T* jp = jamp + __ldg(fm + %d); red_add(jp, ld1<T>(sj + %du * COL)); red_add(jp + BLK, ld1<T>(sj + %du * COL)); }\n"
-                  % (b.slot[f], 2 * sl, 2 * sl + 1))
+                o("    { T* jp = jamp + ldsi(fm + %du); red_add(jp, ld1<T>(sj + %du * COL)); red_add(jp + BLK, ld1<T>(sj + %du * COL)); }\n"
+                  % (4 * b.slot[f], 2 * sl, 2 * sl + 1))
             o("  }\n")
         o("}\n")
         o("__device__ __noinline__ void body%d(%s) {\n  body%d_impl<double>(sinv, tab, sgn, sj, jamp, h, live, fm);\n}\n"
@@ -394,7 +397,7 @@ def emit_coop(n, fp32=True, acc_max=24, **over):
         # per member: gather map of the helicity-independent operands, colour-flow map
         bmeta.append((len(flowmap), len(visits)))
         for pi in fam["members"]:
-            visits.append((len(tabmap), b.ntab, len(invmap), b.ninv, len(ampsign), b.plan.namps))
+            visits.append((len(tabmap), b.ntab, len(invmap), b.ninv, len(ampsign), b.plan.namps, len(flowmap), len(b.flows)))
             for nm, off in sorted(b.inv.items(), key=lambda kv: kv[1]):
                 src = inv[_perm_name(nm, pi)]
                 invmap += [src + j for j in range(b.sizes[nm])]
@@ -412,7 +415,7 @@ def emit_coop(n, fp32=True, acc_max=24, **over):
     algo_slot = gt.flops()           # the tabled currents the diagrams actually use, once per slot
     exec_slot = ftab.flops()         # the kernel builds every current the thresholds allow
     smem = fixed + 2 * nst_used * BLK * 8
-    files.append(_main_unit(E, n, ns, hdr, cfi, cfden, fams, bodies, bmeta, invmap, flowmap, (tabmap, ampsign, visits, namps), ftab,
+    files.append(_main_unit(E, n, ns, hdr, cfi, cfden, fams, bodies, bmeta, invmap, flowmap, (tabmap, ampsign, visits, namps, nflows), ftab,
                             ntabf, inv, ninv, ninvp, ninvs, ntabs, nst_used, fp32, exec_hel + colour_flops, algo + colour_flops,
                             exec_slot, algo_slot, cfg))
     info = dict(proc=proc, ns=ns, npar=npar, ncol=ncol, nhel=nhel, ndiagrams=ndiag,
@@ -449,7 +452,7 @@ def _main_unit(E, n, ns, hdr, cfi, cfden, fams, bodies, bmeta, invmap, flowmap, 
 
     table("inv_map", "short", invmap)
     table("flow_map", "int", flowmap, 16)
-    tabmap, ampsign, visits, namps = tabmaps
+    tabmap, ampsign, visits, namps, nflows = tabmaps
     table("tab_map", "int", tabmap, 24)
     w("__device__ const double amp_sign64[%d] = {\n" % max(1, len(ampsign)))
     for k_ in range(0, len(ampsign), 40):
@@ -462,10 +465,10 @@ def _main_unit(E, n, ns, hdr, cfi, cfden, fams, bodies, bmeta, invmap, flowmap, 
         w("};\n")
         w("MG_DEV const float* amp_sign_of(float*) { return amp_sign32; }\n")
     w("MG_DEV const double* amp_sign_of(double*) { return amp_sign64; }\n")
-    w("constexpr int NVISIT = %d, NAMPS = %d;\n" % (len(visits), namps))
+    w("constexpr int NVISIT = %d, NAMPS = %d, NFLOWS = %d;\n" % (len(visits), namps, nflows))
     w("__constant__ VisitDesc visit_desc[NVISIT + 2] = {\n")
     for v_ in visits:
-        w("  {%d, %d, %d, %d, %d, %d, 0, 0},\n" % v_)
+        w("  {%d, %d, %d, %d, %d, %d, %d, %d},\n" % v_)
     w("  {0, 0, 0, 0, 0, 0, 0, 0}, {0, 0, 0, 0, 0, 0, 0, 0}};\n")
     # helicity-bit shifts per family member: canonical gluon i takes the helicity of gluon pi[i]
     hsh, foff_of = [], {}
@@ -560,11 +563,12 @@ def _main_unit(E, n, ns, hdr, cfi, cfden, fams, bodies, bmeta, invmap, flowmap, 
             "    // body %d: family %s%d, %d terms, %d relabellings\n"
             "#pragma unroll 1\n    for (int m = 0; m < %d; ++m) {\n"
             "      const int v = %d + m;\n"
-            "      visit_step<T, SLOTS>(visit_desc, v, tab_map, inv_map, gtab, asgn, sinv0, sinvp0, smap0, stab0, ssgn0, NINVP, NINVS, NTABS, NTABF, NAMPS);\n"
+            "      visit_step<T, SLOTS>(visit_desc, v, tab_map, inv_map, gtab, asgn, flow_map, sinv0, sinvp0, smap0, stab0, ssgn0, sfm0, NINVP, NINVS,\n"
+            "                           NTABS, NTABF, NAMPS, NFLOWS);\n"
             "      const int hp = permute_helicity<NPAR, NGLU>(h, hel_shift + %d + m * NGLU);\n"
             "      body%d(sinvp, stab0 + (unsigned)(((v & 1) * SLOTS + slot) * NTABS) * SZ, ssgn0 + (unsigned)((v & 1) * NAMPS) * SZ, sj, jamp, hp, live,\n"
-            "             flow_map + %d + m * %d);\n    }\n"
-            % (bi, fams[fi]["kind"], fams[fi]["size"], len(b.plan.terms), nm_, nm_, v0, foff_of[fi], bi, fo, len(b.flows)))
+            "             sfm0 + (unsigned)((v & 1) * NFLOWS) * 4u);\n    }\n"
+            % (bi, fams[fi]["kind"], fams[fi]["size"], len(b.plan.terms), nm_, nm_, v0, foff_of[fi], bi))
     w(KERNEL % dict(calls="".join(calls), minb=cfg.get("ctas_per_sm", 256 // BLK),
                     colour=("T meh;\n    if constexpr (sizeof(T) == 8) {\n"
                             "      colour_dmma_cta<NCOL, BLK>(cf_dense, (const double*)jamp_cta, reinterpret_cast<double*>(smem_raw), (double*)s_meh);\n"
@@ -609,8 +613,8 @@ sigma_kernel(long long nevt, int ntb, int tb_first, const T* __restrict__ lane_w
   // shared memory: full per-event operand set | the running visit's helicity-independent operands | amplitude signs [2] |
   // table operands [2] | index maps [3] | staged JAMPs
   const unsigned sinv0 = sbase, sinvp0 = sinv0 + SLOTS * NINVP * SZ, ssgn0 = sinvp0 + SLOTS * NINVS * SZ;
-  const unsigned stab0 = ssgn0 + 2 * NAMPS * SZ, smap0 = stab0 + 2 * SLOTS * NTABS * SZ;
-  const unsigned sj = smap0 + 3 * NTABS * 4 + ((NTABS & 1) ? 4 : 0) + tid * SZ;
+  const unsigned stab0 = ssgn0 + 2 * NAMPS * SZ, smap0 = stab0 + 2 * SLOTS * NTABS * SZ, sfm0 = smap0 + 3 * NTABS * 4;
+  const unsigned sj = sfm0 + 2 * NFLOWS * 4 + ((NTABS & 1) ? 4 : 0) + tid * SZ;
   const unsigned sinvp = sinvp0 + slot * NINVS * SZ;
   const T* __restrict__ asgn = amp_sign_of((T*)nullptr);
   T* __restrict__ sinv_g = reinterpret_cast<T*>(smem_raw);
@@ -638,7 +642,7 @@ sigma_kernel(long long nevt, int ntb, int tb_first, const T* __restrict__ lane_w
     const int live = slot_live && wgt != T(0);
     __syncthreads();
     build_tables_global<T>(tab_groups, NGROUPS, tab_desc, sinv0, gtab, NINVP, NTABF, SLOTS, s_tbit);
-    visit_prologue<T, SLOTS>(visit_desc, tab_map, gtab, asgn, smap0, stab0, ssgn0, NTABS, NTABF, NAMPS);
+    visit_prologue<T, SLOTS>(visit_desc, tab_map, gtab, asgn, flow_map, smap0, stab0, ssgn0, sfm0, NTABS, NTABF, NAMPS, NFLOWS);
 %(calls)s
     visit_drain();
     __threadfence();                       // the JAMP reductions are performed at L2 before anyone reads them back
@@ -670,7 +674,7 @@ static int run(const double* mom, T* me_out, long long nevt, const T* lane_w, in
   norm /= (double)%(cfden)d * (double)%(denom)d;
   int dev = 0, nsm = 0, per_sm = 0;
   if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return -1;
-  size_t smem = (size_t)(SLOTS * (NINVP + NINVS) + 2 * NAMPS + 2 * SLOTS * NTABS + 2 * NST * BLK) * sizeof(T) + 3 * NTABS * 4 + 8;
+  size_t smem = (size_t)(SLOTS * (NINVP + NINVS) + 2 * NAMPS + 2 * SLOTS * NTABS + 2 * NST * BLK) * sizeof(T) + 3 * NTABS * 4 + 2 * NFLOWS * 4 + 8;
   if (sizeof(T) == 8 && smem < COLOUR_SMEM) smem = COLOUR_SMEM;
   auto kern = sigma_kernel<T>;
   if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return -1;

@@ -506,6 +506,12 @@ def family_key(term, n):
     first block), "Tv3"/"Tk" the big child of the root vertex of a single-block n-gluon tree."""
     ck, fk = group_key(term, n)
     if ck[0] == "T":
+        mid = term[closure_block(term)]
+        sizes = sorted(len(topo.leaves_of(c)) for c in mid[1:])
+        if len(sizes) == 3 and sizes[1] == sizes[2] and sizes[0] < sizes[1]:
+            # gggg root with two equally large children: "the big child" is a tie; the odd one out is unique
+            small = min(mid[1:], key=lambda c: len(topo.leaves_of(c)))
+            return "Tk1", tuple(sorted(topo.leaves_of(small)))
         return "T" + fk[0], fk[1]
     return ck[0], ck[1]
 
