@@ -114,9 +114,9 @@ def build(force=False, log=True, overrides=None):
         objs = list(ex.map(lambda p: _compile(p, force, log), srcs))
     for f in os.listdir(OBJ):            # objects of units that no longer exist
         if f.endswith(".o") and os.path.join(OBJ, f) not in objs:
-            for ext in ("", ".stamp"):
-                if os.path.exists(os.path.join(OBJ, f + ext)):
-                    os.remove(os.path.join(OBJ, f + ext))
+            for victim in (f, f + ".stamp", f[:-2] + ".ptxas.log"):
+                if os.path.exists(os.path.join(OBJ, victim)):
+                    os.remove(os.path.join(OBJ, victim))
     newest = max(os.path.getmtime(o) for o in objs)
     if force or not os.path.exists(LIB) or os.path.getmtime(LIB) < newest:
         cmd = [NVCC] + ARCH + ["-rdc=true", "-shared", "-o", LIB] + objs + ["-lcudart"]
