@@ -238,6 +238,7 @@ int mg_process_destroy(mg_process_t* p) {
   if (!p) return MG_ERR_NULL;
   cudaSetDevice(p->par.device);
   free_all(p);
+  if (cudaCtxResetPersistingL2Cache() != cudaSuccess) (void)cudaGetLastError();   // lines of mg_sigma's L2 window (gg -> t t~ g g g)
   delete p;
   return MG_OK;
 }
