@@ -3,7 +3,7 @@
 # Usage: sh oracle/build.sh   (from anywhere)
 set -e
 cd "$(dirname "$0")"
-SRC="philox_rambo.c lorentz.c colour.c me_eemumu.c me_ggttng.c weight.c"
+SRC="philox_rambo.c lorentz.c colour.c me_eemumu.c me_ggttng.c me_qchannel.c weight.c"
 # -O3 -march=native as SURVEY.md §8(d) states for the timed baseline; -ffp-contract=off keeps the arithmetic of every
 # formula as written (no fused multiply-adds), so results do not depend on the host CPU
 OPT="-O3 -march=native -ffp-contract=off"

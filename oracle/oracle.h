@@ -87,6 +87,15 @@ double oracle_me_ggtt_explicit(const double* p, const oracle_params_t* par);
  * process order: 2 beam gluons then final ones) has its polarisation replaced by its momentum. */
 double oracle_me_ggttng_ward(int nfinal_gluons, const double* p, const oracle_params_t* par, int which);
 
+/* ---- quark channels of p p -> t t~ + jets: top line + one massless quark line of another
+ * flavour + up to 2 gluons, any crossing.  spec: one character per particle in process order ('q' quark, 'Q' antiquark,
+ * 'g' gluon, "tT" at positions 2-3), e.g. "qQtT", "qQtTg", "qgtTq", "gQtTQ", "qQtTgg", "qgtTqg", "ggtTqQ".
+ * Colour-dressed Feynman rules with explicit colour sums (me_qchannel.c).  ward_which >= 0: gluon number ward_which
+ * (in process order among the gluons) has its polarisation replaced by its momentum; -1: physical. ---- */
+double oracle_me_qchannel(const char* spec, const double* p, const oracle_params_t* par, double* hel_out, int ward_which);
+int oracle_me_qchannel_batch(const char* spec, const double* momenta, int64_t nevt, const oracle_params_t* par,
+                             double* me_out, int nthreads);
+
 /* batch drivers (OpenMP over events) for parity and the cpu_baseline timing.
  * proc: 0 = e+e- -> mu+mu-, 1..4 = gg -> tt~ + (proc-1) g.  momenta [nevt][npar][4]. */
 int oracle_me_batch(int proc, const double* momenta, int64_t nevt, const oracle_params_t* par,

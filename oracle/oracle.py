@@ -56,6 +56,9 @@ class Oracle:
         L.oracle_me_ggttng_ward.restype = C.c_double
         L.oracle_rambo.argtypes = [C.c_uint64, C.c_int64, C.c_int64, C.c_int, _dp, C.c_double, _dp, _dp]
         L.oracle_me_batch.argtypes = [C.c_int, _dp, C.c_int64, C.POINTER(Params), _dp, C.c_int]
+        L.oracle_me_qchannel.restype = C.c_double
+        L.oracle_me_qchannel.argtypes = [C.c_char_p, _dp, C.POINTER(Params), _dp, C.c_int]
+        L.oracle_me_qchannel_batch.argtypes = [C.c_char_p, _dp, C.c_int64, C.POINTER(Params), _dp, C.c_int]
         L.oracle_weight_max.argtypes = [_dp, _dp, C.c_int64, C.c_int, _dp, _dp]
 
     def philox(self, ctr, key):
@@ -129,6 +132,22 @@ class Oracle:
         mom = np.ascontiguousarray(momenta, dtype=np.float64)
         out = np.zeros(mom.shape[0])
         rc = self.lib.oracle_me_batch(ip, _p(mom), mom.shape[0], C.byref(par), _p(out), nthreads)
+        assert rc == 0
+        return out
+
+    def me_qchannel(self, spec, p, par=None, per_helicity=False, ward=-1):
+        """Quark channels (oracle.h): spec e.g. "qQtTg"; p [npar][4]."""
+        par = par or default_params(); p = np.ascontiguousarray(p, dtype=np.float64)
+        assert p.shape == (len(spec), 4)
+        hel = np.zeros(1 << len(spec)) if per_helicity else None
+        v = self.lib.oracle_me_qchannel(spec.encode(), _p(p), C.byref(par), _p(hel) if per_helicity else None, C.c_int(ward))
+        return (v, hel) if per_helicity else v
+
+    def me_qchannel_batch(self, spec, momenta, par=None, nthreads=0):
+        par = par or default_params()
+        mom = np.ascontiguousarray(momenta, dtype=np.float64)
+        out = np.zeros(mom.shape[0])
+        rc = self.lib.oracle_me_qchannel_batch(spec.encode(), _p(mom), mom.shape[0], C.byref(par), _p(out), nthreads)
         assert rc == 0
         return out
 

@@ -1,0 +1,150 @@
+"""Pins of the quark-channel oracle (oracle/me_qchannel.c; "pp -> t t~ 0-2 j").
+
+None of these re-types the oracle's recursion:
+  * q q~ -> t t~ against the textbook closed form (Combridge 1979; e.g. Ellis-Stirling-Webber table 10.2)
+        sum-bar |M|^2 = (4 g^4 / 9) [ (m^2 - t)^2 + (m^2 - u)^2 + 2 m^2 s ] / s^2
+    — fixes the absolute normalisation, the spinors of both lines and the colour average;
+  * the Ward identity (polarisation -> momentum gives zero) on every gluon of every process — fixes the relative
+    signs and factors between the diagram classes (emission off either line, three- and four-gluon vertices);
+  * initial-state collinear limits onto that closed form with the Altarelli-Parisi kernels
+        q -> q g :  |M|^2 -> g^2 C_F (1 + x^2)/(1 - x) / (x p_a.k) |M_0(x p_a)|^2
+        g -> q q~:  |M|^2 -> g^2 T_R (x^2 + (1 - x)^2) / (x p_a.k) |M_0(x p_a)|^2
+    — fixes the normalisation of every 1-jet process (incoming-gluon colour and spin averages included), and of the
+    2-jet process q q~ -> t t~ g g against the 1-jet one;
+  * charge conjugation (q <-> q~ together with t <-> t~) and beam exchange.
+"""
+import math
+from concurrent.futures import ThreadPoolExecutor
+
+import numpy as np
+import pytest
+
+from oracle import oracle as O
+
+MT = 173.0
+G2 = 4 * math.pi * 0.118
+CF, TR = 4.0 / 3.0, 0.5
+
+
+@pytest.fixture(scope="module")
+def orc():
+    return O.Oracle()
+
+
+def mdot(a, b):
+    return a[0] * b[0] - a[1] * b[1] - a[2] * b[2] - a[3] * b[3]
+
+
+def born_closed_form(pa, pb, pt):
+    s = mdot(pa + pb, pa + pb)
+    t = mdot(pa - pt, pa - pt)
+    u = 2 * MT * MT - s - t
+    return 4 * G2 * G2 / 9 * ((MT * MT - t) ** 2 + (MT * MT - u) ** 2 + 2 * MT * MT * s) / s ** 2
+
+
+def test_qqbar_to_ttbar_equals_the_closed_form(orc):
+    mom = orc.rambo(11, 16, [MT, MT], 1500.0)
+    for p in mom:
+        ref = born_closed_form(p[0], p[1], p[2])
+        assert abs(orc.me_qchannel("qQtT", p) / ref - 1) < 1e-12
+        # antiquark in the first beam: the same formula with the beams exchanged
+        assert abs(orc.me_qchannel("QqtT", p) / born_closed_form(p[1], p[0], p[2]) - 1) < 1e-12
+
+
+@pytest.mark.parametrize("spec", ["qQtTg", "QqtTg", "qgtTq", "gqtTq", "QgtTQ", "gQtTQ"])
+def test_ward_identity_one_jet(orc, spec):
+    mom = orc.rambo(12, 3, [MT, MT, 0.0], 1500.0)
+    for p in mom:
+        v = orc.me_qchannel(spec, p)
+        assert v > 0
+        assert orc.me_qchannel(spec, p, ward=0) / v < 1e-20
+
+
+def test_ward_identity_two_jets(orc):
+    p = orc.rambo(13, 1, [MT, MT, 0.0, 0.0], 1500.0)[0]
+    jobs = [(spec, w) for spec in ("qQtTgg", "qgtTqg", "ggtTqQ") for w in (-1, 0, 1)]
+    with ThreadPoolExecutor(9) as ex:
+        res = dict(zip(jobs, ex.map(lambda j: orc.me_qchannel(j[0], p, ward=j[1]), jobs)))
+    for spec in ("qQtTgg", "qgtTqg", "ggtTqQ"):
+        assert res[(spec, -1)] > 0
+        for w in (0, 1):
+            assert res[(spec, w)] / res[(spec, -1)] < 1e-20
+
+
+def _boost(p, Q):
+    M = math.sqrt(mdot(Q, Q))
+    b = Q[1:] / Q[0]
+    g = Q[0] / M
+    bp = b @ p[1:]
+    out = np.zeros(4)
+    out[0] = g * (p[0] + bp)
+    out[1:] = p[1:] + ((g - 1) * bp / (b @ b) + g * p[0]) * b
+    return out
+
+
+def _collinear_event(x, theta, beam, E=750.0, extra=None):
+    """2 -> t t~ + k (+ extra) with k = (1 - x) * beam momentum, tilted by theta; momentum conserved exactly."""
+    pa = np.array([E, 0, 0, E])
+    pb = np.array([E, 0, 0, -E])
+    sgn = 1 if beam == 0 else -1
+    k = (1 - x) * E * np.array([1, math.sin(theta) * math.cos(0.7), math.sin(theta) * math.sin(0.7), sgn * math.cos(theta)])
+    Q = pa + pb - k
+    if extra is not None:
+        Q = Q - extra
+    M = math.sqrt(mdot(Q, Q))
+    pp = math.sqrt(M * M / 4 - MT * MT)
+    ct, ph = 0.3, 1.1
+    st = math.sqrt(1 - ct * ct)
+    t = np.array([M / 2, pp * st * math.cos(ph), pp * st * math.sin(ph), pp * ct])
+    tb = np.array([M / 2, -t[1], -t[2], -t[3]])
+    return pa, pb, _boost(t, Q), _boost(tb, Q), k
+
+
+@pytest.mark.parametrize("x", [0.6, 0.8])
+def test_initial_state_collinear_limits_onto_the_closed_form(orc, x):
+    err = {}
+    for theta in (1e-2, 1e-3):
+        pa, pb, t, tb, k = _collinear_event(x, theta, 0)
+        p = np.array([pa, pb, t, tb, k])
+        r1 = orc.me_qchannel("qQtTg", p) / (G2 * CF * (1 + x * x) / (1 - x) / (x * mdot(pa, k)) * born_closed_form(x * pa, pb, t))
+        r3 = orc.me_qchannel("gQtTQ", p) / (G2 * TR * (x * x + (1 - x) ** 2) / (x * mdot(pa, k)) * born_closed_form(x * pa, pb, t))
+        pa, pb, t, tb, k = _collinear_event(x, theta, 1)
+        p = np.array([pa, pb, t, tb, k])
+        r2 = orc.me_qchannel("qgtTq", p) / (G2 * TR * (x * x + (1 - x) ** 2) / (x * mdot(pb, k)) * born_closed_form(pa, x * pb, t))
+        err[theta] = [abs(r - 1) for r in (r1, r2, r3)]
+    assert max(err[1e-3]) < 2e-3
+    for a, b in zip(err[1e-2], err[1e-3]):        # the correction is linear in the angle
+        assert b < 0.2 * a
+
+
+def test_two_jet_collinear_limit_onto_the_one_jet_process(orc):
+    x = 0.7
+    g1 = np.array([120.0, 60.0, -80.0, 66.332495807108])        # a hard, well-separated massless gluon
+    g1[0] = math.sqrt(g1[1] ** 2 + g1[2] ** 2 + g1[3] ** 2)
+
+    def ratio(theta):
+        pa, pb, t, tb, k = _collinear_event(x, theta, 0, extra=g1)
+        v = orc.me_qchannel("qQtTgg", np.array([pa, pb, t, tb, g1, k]))
+        ref = orc.me_qchannel("qQtTg", np.array([x * pa, pb, t, tb, g1]))
+        # the identical-gluon factor 1/2 of the 2-jet process: the collinear gluon is one specific gluon of the two
+        return 2 * v / (G2 * CF * (1 + x * x) / (1 - x) / (x * mdot(pa, k)) * ref)
+
+    with ThreadPoolExecutor(2) as ex:
+        r2, r3 = ex.map(ratio, (1e-2, 1e-3))
+    assert abs(r3 - 1) < 3e-3 and abs(r3 - 1) < 0.2 * abs(r2 - 1)
+
+
+def test_charge_conjugation_and_beam_exchange(orc):
+    mom = orc.rambo(14, 3, [MT, MT, 0.0], 1500.0)
+    for p in mom:
+        c = p[[0, 1, 3, 2, 4]]                   # t <-> t~
+        assert abs(orc.me_qchannel("qQtTg", p) / orc.me_qchannel("QqtTg", c) - 1) < 1e-10
+        assert abs(orc.me_qchannel("qgtTq", p) / orc.me_qchannel("QgtTQ", c) - 1) < 1e-10
+        b = p[[1, 0, 2, 3, 4]]                   # beams exchanged
+        assert abs(orc.me_qchannel("qgtTq", p) / orc.me_qchannel("gqtTq", b) - 1) < 1e-10
+
+
+def test_bad_specs_are_rejected(orc):
+    p = np.zeros((5, 4))
+    for spec in ("qqtTg", "qQTtg", "ggtTg", "qQtTq"):
+        assert orc.me_qchannel(spec, p) == -1
