@@ -32,6 +32,7 @@ def generate(overrides=None):
     (tuning runs only): {n_gluons: dict of emit_coop keyword overrides}."""
     import json
     from .gen.emit import emit_eemumu, emit_ggttng
+    from .gen.quark import SPECS, emit_quark
     os.makedirs(GEN, exist_ok=True)
     infos, paths = [], []
     jobs = [emit_eemumu()]
@@ -39,6 +40,8 @@ def generate(overrides=None):
         kw = dict(fp32=(n < 5))
         kw.update((overrides or {}).get(n, {}))
         jobs.append(emit_ggttng(n, **kw))
+    for spec in SPECS:                       # quark channels of p p -> t t~ + 0..2 jets
+        jobs.append(emit_quark(spec))
     keep = set()
     for files, info in jobs:
         for fname, src in files:

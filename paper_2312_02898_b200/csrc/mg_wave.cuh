@@ -332,6 +332,15 @@ template <class T> MG_DEV void bilinear(const W4<T>& L, const W4<T>& R, W4<T>& B
   B.r[2] = -zi;
   B.i[2] = zr;
 }
+// quark pair -> off-shell gluon (quark channels, gen/quark.py):  j^mu = s * L gamma^mu R  (index raised), s = -1/P^2
+template <class T> MG_DEV void cur_pair(const W4<T>& L, const W4<T>& R, T s, W4<T>& o) {
+  W4<T> B;
+  bilinear(L, R, B);
+  o.r[0] = s * B.r[0];
+  o.i[0] = s * B.i[0];
+#pragma unroll
+  for (int m = 1; m < 4; ++m) { o.r[m] = -s * B.r[m]; o.i[m] = -s * B.i[m]; }
+}
 // plain (already index-lowered) contraction  sum_mu B_mu j^mu
 template <class T> MG_DEV C1<T> contract(const W4<T>& B, const W4<T>& j) {
   C1<T> d;

@@ -1,0 +1,106 @@
+"""GPU parity of the quark channels of p p -> t t~ + 0..2 jets: the generated fused
+kernels (gen/quark.py), called through the C ABI, against the colour-dressed oracle (oracle/me_qchannel.c) on the
+momenta the CUDA RAMBO generated.  Same bound as the gluon channels (tests/test_gpu_parity.py, reading A12).
+"""
+import numpy as np
+import pytest
+
+import workloads
+from test_gpu_parity import TOL32_MAX, TOL32_MED, gpu_events, parity_bound, report
+
+pytestmark = pytest.mark.gpu
+
+# events per subprocess: the oracle costs ~2 ms (0 jets), 0.1 s (1 jet), 5 s (2 jets) per event and core
+NEVT = {4: 4133, 5: 1029, 6: 37}
+
+
+@pytest.fixture(scope="module")
+def mg():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    import paper_2312_02898_b200 as m
+    m.lib()
+    return m
+
+
+@pytest.mark.parametrize("spec", workloads.QUARK_SPECS)
+def test_quark_channel_fp64_parity(mg, oracle, oracle_ld, spec):
+    import torch
+    cfg = workloads.QUARK_CHANNELS[spec]
+    nevt = NEVT[len(spec)]
+    ref = None
+    for mode in (mg.HEL_ALL, mg.HEL_FILTER):
+        proc = mg.Process(cfg["proc"], helicity_mode=mode)
+        assert proc.info.npar == len(spec)
+        mom, ev = gpu_events(mg, proc, cfg, nevt)
+        me = proc.sigma(mom, nevt)
+        torch.cuda.synchronize()
+        me = me.cpu().numpy()
+        if ref is None:
+            orc = oracle_ld if len(spec) < 6 else oracle          # the long-double build is 4x slower: 2-jet events use double
+            ref = orc.me_qchannel_batch(spec, ev)
+        rel = np.abs(me / ref - 1)
+        bound = parity_bound(ev, cfg["sqrt_s"])
+        rec = report("quark %s mode %d" % (spec, mode), rel, bound)
+        assert np.all(np.isfinite(me)) and np.all(me > 0)
+        assert rec["above_bound"] == 0, (spec, mode, rel.max(), int(rel.argmax()))
+        assert rec["median"] < 1e-12
+        proc.close()
+
+
+@pytest.mark.parametrize("spec", ["qQtTg", "gQtTQ", "qgtTqg"])
+def test_quark_channel_per_helicity_and_filter(mg, oracle, spec):
+    """Per-helicity |M_h|^2 against the oracle's, and the helicity bookkeeping: chirality conservation along the massless
+    line halves the good helicities, the helicity-flip symmetry halves the evaluated ones again."""
+    import torch
+    cfg = workloads.QUARK_CHANNELS[spec]
+    nevt = 8 if len(spec) == 6 else 64
+    proc = mg.Process(cfg["proc"])
+    mom, ev = gpu_events(mg, proc, cfg, nevt)
+    proc.helicity_probe(mom, nevt)
+    info = proc.info
+    assert info.nhel == 1 << len(spec)
+    assert info.ngoodhel == info.nhel // 2
+    assert info.nhel_evaluated == info.nhel // 4
+    ph = proc.sigma_per_helicity(mom, nevt)
+    torch.cuda.synchronize()
+    ph = ph.cpu().numpy()
+    for e in range(min(nevt, 4)):
+        tot, hel = oracle.me_qchannel(spec, ev[e], per_helicity=True)
+        scale = hel.max()
+        assert np.abs(ph[:, e] - hel).max() < 1e-9 * scale
+    proc.close()
+
+
+@pytest.mark.parametrize("spec", ["qQtTg", "qgtTqg"])
+def test_quark_channel_fp32(mg, oracle, spec):
+    import torch
+    cfg = workloads.QUARK_CHANNELS[spec]
+    nevt = 4133
+    p64 = mg.Process(cfg["proc"])
+    p32 = mg.Process(cfg["proc"], precision=mg.FP32)
+    mom, ev = gpu_events(mg, p64, cfg, nevt)
+    a = p64.sigma(mom, nevt).cpu().numpy()
+    b = p32.sigma(mom, nevt).cpu().numpy().astype(np.float64)
+    torch.cuda.synchronize()
+    rel = np.abs(b / a - 1)
+    assert np.median(rel) < TOL32_MED and rel.max() < TOL32_MAX, (np.median(rel), rel.max())
+    p64.close()
+    p32.close()
+
+
+def test_subprocess_sum_of_one_event_batch(mg, oracle):
+    """Several subprocesses evaluated on the SAME momenta (what a p p -> t t~ j event needs before the PDFs weight them):
+    one handle per subprocess, one momenta buffer."""
+    import torch
+    specs = ["qQtTg", "QqtTg", "qgtTq", "gqtTq", "QgtTQ", "gQtTQ"]
+    cfg = workloads.QUARK_CHANNELS[specs[0]]
+    procs = [mg.Process(workloads.QUARK_CHANNELS[s]["proc"]) for s in specs]
+    nevt = 256
+    mom, ev = gpu_events(mg, procs[0], cfg, nevt)
+    for s, p in zip(specs, procs):
+        me = p.sigma(mom, nevt)
+        torch.cuda.synchronize()
+        ref = oracle.me_qchannel_batch(s, ev)
+        assert np.abs(me.cpu().numpy() / ref - 1).max() < 1e-9
+        p.close()
