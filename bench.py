@@ -35,7 +35,10 @@ def parse():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--workload", default="ggttgg", choices=list(workloads.CONFIGS))
+    ap.add_argument("--workload", default="ggttgg",
+                    choices=list(workloads.CONFIGS) + ["quark_" + q for q in workloads.QUARK_SPECS],
+                    help="a BASELINE.json config, or quark_<spec>: one quark channel of p p > t t~ + jets (SURVEY 8f-3; not a "
+                         "BASELINE.json config: reported for the record, no cpu_baseline leg)")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--precision", default="fp64", choices=["fp64", "fp32"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -45,8 +48,9 @@ def parse():
 
 
 def config_dict(name, cfg, world, precision):
-    return {"workload": "%s: %s, sqrt_s=%g GeV, %d RAMBO events/GPU, Philox seed %d (BASELINE.json configs[%d])"
-                        % (name, cfg["proc"], cfg["sqrt_s"], cfg["nevt"], cfg["seed"], cfg["index"]),
+    where = "BASELINE.json configs[%d]" % cfg["index"] if cfg["index"] >= 0 else "not a BASELINE.json config"
+    return {"workload": "%s: %s, sqrt_s=%g GeV, %d RAMBO events/GPU, Philox seed %d (%s)"
+                        % (name, cfg["proc"], cfg["sqrt_s"], cfg["nevt"], cfg["seed"], where),
             "proc": cfg["proc"], "nevt_per_gpu": cfg["nevt"], "global_batch": cfg["nevt"] * world,
             "sqrt_s": cfg["sqrt_s"], "seed": cfg["seed"], "precision": precision,
             "parallelism": "events sharded over %d GPU(s), no collective" % world,
@@ -323,7 +327,14 @@ def measure(mg, torch, dist, name, cfg, args, steps, rank, world, local, peaks, 
 def main():
     args = parse()
     name = args.workload
-    cfg = dict(workloads.CONFIGS[name])
+    if name.startswith("quark_"):
+        cfg = dict(workloads.QUARK_CHANNELS[name[6:]], nevt=524288, index=-1)
+        args.single = args.no_cpu_baseline = True
+        if args.impl == "reference":
+            print(json.dumps({"impl": "reference", "unavailable": "the reference arm times the BASELINE.json configs only"}))
+            return 0
+    else:
+        cfg = dict(workloads.CONFIGS[name])
     if args.nevt:
         cfg["nevt"] = args.nevt
     if args.impl == "reference":

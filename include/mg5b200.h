@@ -6,7 +6,10 @@
  * :41, :45).  The caller owns batches; the library is a pure function momenta -> |M|^2 (the shape of the
  * Fortran<->CUDA bridge of PAPER.md:67-:89, Fig. 1c).  Processes: the set validated in PAPER.md:139 —
  *     "e+ e- > mu+ mu-", "g g > t t~", "g g > t t~ g", "g g > t t~ g g", "g g > t t~ g g g"
- * (leading order, fixed couplings: PAPER.md:141).
+ * (leading order, fixed couplings: PAPER.md:141), and the quark channels of p p > t t~ + 0..2 jets that have one
+ * light-quark line ("p p -> t t~ 0-2 j"; q = one massless flavour other than the top):
+ *     "q q~ > t t~ [g [g]]", "q~ q > t t~ [g [g]]", "q g > t t~ q [g]", "g q > t t~ q [g]", "q~ g > t t~ q~ [g]",
+ *     "g q~ > t t~ q~ [g]", "g g > t t~ q q~";   several subprocesses behind one handle: mg_multi_* below.
  *
  * Plain C: opaque handle, plain pointers and sizes.  Every `*_dev` pointer is DEVICE memory owned by the
  * caller (the library never frees or reallocates it); `stream` is a cudaStream_t passed as void* (NULL =
@@ -19,7 +22,8 @@
  * particles in the order of the process string (initial state first).  nevt need not be a multiple of 32
  * but the buffer must be mg_momenta_bytes(p, nevt) long (whole pages) and 16-byte aligned.
  * Output: me_out[nevt], double (MG_FP64) or float (MG_FP32): spin- and colour-averaged |M|^2 including the
- * 1/k! for k identical final-state gluons (denominators 4, 256, 256, 512, 1536), in GeV^(-2(npar-4)).
+ * 1/k! for k identical final-state gluons (denominators 4, 256, 256, 512, 1536 for the five processes of PAPER.md:139;
+ * 36 / 96 / 256 x k! for q q~ / q g / g g beams in the quark channels), in GeV^(-2(npar-4)).
  */
 #ifndef MG5B200_H
 #define MG5B200_H
@@ -36,7 +40,7 @@ typedef struct mg_process mg_process_t; /* opaque, library-owned */
 typedef enum {
   MG_OK = 0,
   MG_ERR_NULL = -1,       /* a required pointer argument is NULL                       */
-  MG_ERR_BAD_PROC = -2,   /* process string not one of the five generated processes    */
+  MG_ERR_BAD_PROC = -2,   /* process string not one of the generated processes         */
   MG_ERR_BAD_PARAM = -3,  /* struct_size mismatch, unknown precision / helicity mode   */
   MG_ERR_BAD_NEVT = -4,   /* nevt < 0                                                  */
   MG_ERR_ALIGN = -5,      /* a device pointer is not 16-byte aligned                   */
@@ -147,7 +151,6 @@ int mg_helicity_probe(mg_process_t* p, const void* momenta_dev, int64_t nprobe, 
  * perhel_out_dev[h * nevt + ievt].  Diagnostic / test entry point. */
 int mg_sigma_per_helicity(mg_process_t* p, const void* momenta_dev, int64_t nevt, void* perhel_out_dev,
                           void* stream);
-/* Copies the current good-helicity list (indices; bit (npar-1-i) set <=> particle i has lambda=+1). */
 /* Mixed precision with precision tracking ("tracking the precision of the matrix elements
  * showed that single-precision computations are not accurate enough"): on an MG_FP64 handle of a process that has fp32
  * kernels (all but g g > t t~ g g g), evaluates every helicity in fp32, measures per event
@@ -162,7 +165,27 @@ int mg_sigma_per_helicity(mg_process_t* p, const void* momenta_dev, int64_t nevt
 int mg_sigma_mixed(mg_process_t* p, const void* momenta_dev, int64_t nevt, double* me_out_dev, double tol,
                    float* eps_out_dev, int64_t* nflagged_out, void* stream);
 
+/* Copies the current good-helicity list (indices; bit (npar-1-i) set <=> particle i has lambda=+1). */
 int mg_good_helicities(const mg_process_t* p, int32_t* out, int32_t capacity, int32_t* ngood);
+
+/* Several subprocesses behind one handle ("Processes with multiple subprocesses, such as
+ * proton-proton collisions p p -> t t~ 0-2 j ... are being tested").  `proc` may use the multi-particle labels p (beams)
+ * and j (jets) = {g, q, q~} (q: one massless quark flavour other than the top), e.g. "p p > t t~ j": it is expanded to
+ * every combination, the jets as a multiset, and the combinations for which a subprocess exists are kept — the gluon
+ * channels g g > t t~ (g (g)) and the 15 subprocesses with one light-quark line (q q~ > t t~ g, q g > t t~ q, ...,
+ * g g > t t~ q q~).  NOT generated: the 2-jet subprocesses with two light-quark lines (q q~ > t t~ q' q'~, q q' > t t~ q q',
+ * ...); mg_multi_name lists what the handle holds.  MG_ERR_BAD_PROC if nothing matches.
+ * mg_multi_sigma: |M|^2 of every subprocess on the SAME nevt momenta (all share npar and the momenta layout);
+ * me_out_dev[isub * nevt + ievt], element type of the precision.  PDFs and the sum over subprocesses stay with the caller
+ * (host side).  mg_multi_process returns the borrowed single-subprocess handle (owned by the multi handle)
+ * for mg_rambo, mg_process_info, mg_helicity_probe etc.  Same stream / ordering rules as mg_sigma. */
+typedef struct mg_multi mg_multi_t;
+int mg_multi_create(const char* proc, const mg_params_t* params, mg_multi_t** out);
+int mg_multi_destroy(mg_multi_t* m);
+int mg_multi_count(const mg_multi_t* m);
+const char* mg_multi_name(const mg_multi_t* m, int isub);
+mg_process_t* mg_multi_process(mg_multi_t* m, int isub);
+int mg_multi_sigma(mg_multi_t* m, const void* momenta_dev, int64_t nevt, void* me_out_dev, void* stream);
 
 int mg_process_info(const mg_process_t* p, mg_info_t* out);
 size_t mg_momenta_bytes(const mg_process_t* p, int64_t nevt);

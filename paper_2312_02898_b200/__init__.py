@@ -20,7 +20,8 @@ HEL_FILTER, HEL_ALL = 0, 1
 
 SYMBOLS = ["mg_params_default", "mg_process_create", "mg_process_destroy", "mg_rambo", "mg_rambo_ex", "mg_philox_raw", "mg_sigma",
            "mg_sigma_host", "mg_helicity_probe", "mg_sigma_per_helicity", "mg_good_helicities", "mg_process_info",
-           "mg_momenta_bytes", "mg_set_workspace", "mg_workspace_bytes", "mg_weight_max", "mg_sigma_mixed", "mg_status_string", "mg_last_error"]
+           "mg_momenta_bytes", "mg_set_workspace", "mg_workspace_bytes", "mg_weight_max", "mg_sigma_mixed", "mg_status_string", "mg_last_error",
+           "mg_multi_create", "mg_multi_destroy", "mg_multi_count", "mg_multi_name", "mg_multi_process", "mg_multi_sigma"]
 
 
 class MgParams(C.Structure):
@@ -75,6 +76,14 @@ def lib():
         L.mg_workspace_bytes.restype = C.c_size_t
         L.mg_weight_max.argtypes = [vp, vp, vp, i64, vp, vp]
         L.mg_sigma_mixed.argtypes = [vp, vp, i64, vp, C.c_double, vp, C.POINTER(i64), vp]
+        L.mg_multi_create.argtypes = [C.c_char_p, C.POINTER(MgParams), C.POINTER(vp)]
+        L.mg_multi_destroy.argtypes = [vp]
+        L.mg_multi_count.argtypes = [vp]
+        L.mg_multi_name.argtypes = [vp, C.c_int]
+        L.mg_multi_name.restype = C.c_char_p
+        L.mg_multi_process.argtypes = [vp, C.c_int]
+        L.mg_multi_process.restype = vp
+        L.mg_multi_sigma.argtypes = [vp, vp, i64, vp, vp]
         L.mg_status_string.argtypes = [C.c_int]
         L.mg_status_string.restype = C.c_char_p
         L.mg_last_error.restype = C.c_char_p
@@ -230,6 +239,50 @@ class Process:
         buf = (C.c_int32 * 256)()
         _check(lib().mg_good_helicities(self._h, buf, 256, C.byref(n)))
         return [int(buf[i]) for i in range(n.value)]
+
+
+class MultiProcess:
+    """Several subprocesses behind one handle (mg_multi_t): "p p > t t~ j" etc.; `sub[i]` are borrowed Process views."""
+
+    def __init__(self, proc, precision=FP64, helicity_mode=HEL_FILTER, device=0, **params):
+        self._m = C.c_void_p()
+        self.params = default_params(precision, helicity_mode, device, **params)
+        _check(lib().mg_multi_create(proc.encode(), C.byref(self.params), C.byref(self._m)))
+        self.precision, self.device = precision, device
+        n = lib().mg_multi_count(self._m)
+        self.names = [lib().mg_multi_name(self._m, i).decode() for i in range(n)]
+        self.sub = []
+        for i in range(n):
+            v = Process.__new__(Process)          # a view: the multi handle owns the subprocess handle
+            v._h = None
+            v._borrowed = C.c_void_p(lib().mg_multi_process(self._m, i))
+            v.params, v.proc, v.precision, v.device = self.params, self.names[i], precision, device
+            self.sub.append(v)
+        for v in self.sub:
+            v._h = v._borrowed
+            v.close = lambda: None                # never destroyed through the view
+
+    def sigma(self, momenta, nevt, out=None, stream=None):
+        """|M|^2 of every subprocess on the same momenta: tensor [nsub][nevt]."""
+        import torch
+        if out is None:
+            out = torch.empty((len(self.sub), nevt), dtype=torch.float64 if self.precision == FP64 else torch.float32,
+                              device=momenta.device)
+        _check(lib().mg_multi_sigma(self._m, C.c_void_p(momenta.data_ptr()), nevt, C.c_void_p(out.data_ptr()), _stream_ptr(stream)))
+        return out
+
+    def close(self):
+        if getattr(self, "_m", None) is not None and self._m.value:
+            for v in self.sub:
+                v._h = C.c_void_p()
+            lib().mg_multi_destroy(self._m)
+            self._m = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
 
 
 def shard(nevt_per_gpu, rank, world_size=1):

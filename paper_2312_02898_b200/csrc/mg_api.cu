@@ -494,6 +494,95 @@ int mg_process_info(const mg_process_t* p, mg_info_t* o) {
   return MG_OK;
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// Several subprocesses behind one handle ("processes with multiple subprocesses, such as p p -> t t~ 0-2 j").
+// `p` (beams) and `j` (jets) stand for {g, q, q~}; the string is expanded to every combination, jets as a multiset, and
+// the combinations for which a subprocess was generated are kept (quark number is conserved by construction: the others
+// do not exist).  All subprocesses share npar, hence one momenta buffer.
+// ---------------------------------------------------------------------------------------------------------------
+struct mg_multi {
+  std::vector<mg_process*> sub;
+  std::vector<std::string> names;
+};
+
+static const mg_procdesc_t* find_desc(const std::string& key) {
+  for (int i = 0; i < mg_registry_n; ++i) if (squeeze(mg_registry[i]->proc) == key) return mg_registry[i];
+  return nullptr;
+}
+
+int mg_multi_create(const char* proc, const mg_params_t* params, mg_multi_t** out) {
+  if (!proc || !params || !out) return MG_ERR_NULL;
+  std::vector<std::string> ini, fin;
+  {
+    std::vector<std::string>* cur = &ini;
+    std::string tok;
+    for (const char* c = proc;; ++c) {
+      if (*c == 0 || isspace((unsigned char)*c) || *c == '>') {
+        if (!tok.empty()) { cur->push_back(tok); tok.clear(); }
+        if (*c == '>') { if (cur == &fin) return MG_ERR_BAD_PROC; cur = &fin; }
+        if (*c == 0) break;
+      } else tok.push_back(*c);
+    }
+  }
+  if (ini.size() != 2 || fin.size() < 2 || fin.size() > 6) return MG_ERR_BAD_PROC;
+  static const char* const parton[3] = {"g", "q", "q~"};
+  std::vector<int> jets;                           // positions of the j's in the final state
+  for (size_t i = 0; i < fin.size(); ++i) if (fin[i] == "j") jets.push_back((int)i);
+  const int nj = (int)jets.size();
+  int ncomb = 1;
+  for (int i = 0; i < nj; ++i) ncomb *= 3;
+  mg_multi* m = new mg_multi();
+  int rc = MG_OK;
+  for (int a = 0; a < 3 && rc == MG_OK; ++a) {
+    if (ini[0] != "p" && a > 0) break;
+    for (int b = 0; b < 3 && rc == MG_OK; ++b) {
+      if (ini[1] != "p" && b > 0) break;
+      for (int c = 0; c < ncomb && rc == MG_OK; ++c) {
+        std::vector<std::string> f = fin;
+        int r = c;
+        for (int i = 0; i < nj; ++i) { f[jets[i]] = parton[r % 3]; r /= 3; }
+        std::string name = std::string(ini[0] == "p" ? parton[a] : ini[0].c_str()) + " " +
+                           (ini[1] == "p" ? parton[b] : ini[1].c_str()) + " >";
+        for (const std::string& t : f) name += " " + t;
+        const mg_procdesc_t* d = find_desc(squeeze(name.c_str()));
+        if (!d) continue;                          // jets in another order, or no such subprocess
+        bool dup = false;
+        for (const mg_process* q : m->sub) if (q->desc == d) dup = true;
+        if (dup) continue;
+        mg_process* h = nullptr;
+        rc = mg_process_create(d->proc, params, &h);
+        if (rc == MG_OK) { m->sub.push_back(h); m->names.push_back(d->proc); }
+      }
+    }
+  }
+  if (rc == MG_OK && m->sub.empty()) rc = MG_ERR_BAD_PROC;
+  if (rc != MG_OK) { mg_multi_destroy(m); return rc; }
+  *out = m;
+  return MG_OK;
+}
+
+int mg_multi_destroy(mg_multi_t* m) {
+  if (!m) return MG_ERR_NULL;
+  for (mg_process* h : m->sub) mg_process_destroy(h);
+  delete m;
+  return MG_OK;
+}
+
+int mg_multi_count(const mg_multi_t* m) { return m ? (int)m->sub.size() : 0; }
+const char* mg_multi_name(const mg_multi_t* m, int i) { return (m && i >= 0 && i < (int)m->sub.size()) ? m->names[i].c_str() : nullptr; }
+mg_process_t* mg_multi_process(mg_multi_t* m, int i) { return (m && i >= 0 && i < (int)m->sub.size()) ? m->sub[i] : nullptr; }
+
+int mg_multi_sigma(mg_multi_t* m, const void* momenta_dev, int64_t nevt, void* me_out_dev, void* stream) {
+  if (!m || ((!momenta_dev || !me_out_dev) && nevt > 0)) return MG_ERR_NULL;
+  if (nevt < 0) return MG_ERR_BAD_NEVT;
+  for (size_t i = 0; i < m->sub.size(); ++i) {
+    char* out = (char*)me_out_dev + i * (size_t)nevt * esize(m->sub[i]);
+    const int rc = mg_sigma(m->sub[i], momenta_dev, nevt, out, stream);
+    if (rc != MG_OK) return rc;
+  }
+  return MG_OK;
+}
+
 const char* mg_status_string(int s) {
   switch (s) {
     case MG_OK: return "ok";

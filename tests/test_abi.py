@@ -51,6 +51,9 @@ def test_status_strings_and_argument_errors_without_gpu():
     h = C.c_void_p()
     p = mg.default_params()
     assert L.mg_process_create(b"u u~ > d d~", C.byref(p), C.byref(h)) == -2      # MG_ERR_BAD_PROC
+    assert L.mg_multi_create(b"p p > b b~ j", C.byref(p), C.byref(h)) == -2        # nothing generated matches
+    assert L.mg_multi_create(b"p p > t t~ > j", C.byref(p), C.byref(h)) == -2
+    assert L.mg_multi_count(None) == 0 and L.mg_multi_sigma(None, None, 0, None, None) == -1
     p.struct_size = 12
     assert L.mg_process_create(b"g g > t t~", C.byref(p), C.byref(h)) == -3       # MG_ERR_BAD_PARAM
     p = mg.default_params(gamma_t=1.5)

@@ -89,18 +89,25 @@ def test_quark_channel_fp32(mg, oracle, spec):
     p32.close()
 
 
-def test_subprocess_sum_of_one_event_batch(mg, oracle):
-    """Several subprocesses evaluated on the SAME momenta (what a p p -> t t~ j event needs before the PDFs weight them):
-    one handle per subprocess, one momenta buffer."""
+@pytest.mark.parametrize("proc,nsub,nevt", [("p p > t t~", 3, 512), ("p p > t t~ j", 7, 256), ("p p > t t~ j j", 8, 16)])
+def test_multi_subprocess_handle(mg, oracle, proc, nsub, nevt):
+    """Several subprocesses behind one handle, evaluated on the SAME momenta (what a p p -> t t~ + jets event needs before
+    the PDFs weight them): every row against the oracle of its subprocess."""
     import torch
-    specs = ["qQtTg", "QqtTg", "qgtTq", "gqtTq", "QgtTQ", "gQtTQ"]
-    cfg = workloads.QUARK_CHANNELS[specs[0]]
-    procs = [mg.Process(workloads.QUARK_CHANNELS[s]["proc"]) for s in specs]
-    nevt = 256
-    mom, ev = gpu_events(mg, procs[0], cfg, nevt)
-    for s, p in zip(specs, procs):
-        me = p.sigma(mom, nevt)
-        torch.cuda.synchronize()
-        ref = oracle.me_qchannel_batch(s, ev)
-        assert np.abs(me.cpu().numpy() / ref - 1).max() < 1e-9
-        p.close()
+    m = mg.MultiProcess(proc)
+    assert len(m.names) == nsub == len(set(m.names))
+    spec_of = {v["proc"]: k for k, v in workloads.QUARK_CHANNELS.items()}
+    cfg = dict(sqrt_s=1500.0, seed=77)
+    mom, ev = gpu_events(mg, m.sub[0], cfg, nevt)
+    me = m.sigma(mom, nevt)
+    torch.cuda.synchronize()
+    me = me.cpu().numpy()
+    assert me.shape == (nsub, nevt)
+    for i, name in enumerate(m.names):
+        ref = oracle.me_qchannel_batch(spec_of[name], ev) if name in spec_of else oracle.me_batch(name, ev)
+        assert np.abs(me[i] / ref - 1).max() < 1e-9, name
+        assert m.sub[i].info.npar == ev.shape[1]
+    m.close()
+    with pytest.raises(mg.MgError) as err:
+        mg.MultiProcess("p p > b b~ j")
+    assert err.value.status == -2
