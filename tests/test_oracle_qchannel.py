@@ -11,7 +11,14 @@ None of these re-types the oracle's recursion:
         g -> q q~:  |M|^2 -> g^2 T_R (x^2 + (1 - x)^2) / (x p_a.k) |M_0(x p_a)|^2
     — fixes the normalisation of every 1-jet process (incoming-gluon colour and spin averages included), and of the
     2-jet process q q~ -> t t~ g g against the 1-jet one;
-  * charge conjugation (q <-> q~ together with t <-> t~) and beam exchange.
+  * charge conjugation (q <-> q~ together with t <-> t~) and beam exchange;
+  * two light-quark lines (flavours q and r): the final-state collinear limit r r~ -> g of q q~ -> t t~ r r~ onto
+    q q~ -> t t~ g with <P_qg> = T_R (1 - 2 z (1 - z)) (two azimuths pi/2 apart cancel the spin correlation), the
+    initial-state limit q -> g q of q r -> t t~ q r onto g r -> t t~ r with P_gq = C_F (1 + (1 - x)^2)/x, and the
+    relabelling symmetries.  Same flavour twice (q q~ -> t t~ q q~, q q -> t t~ q q): the amplitude is the difference of the
+    two ways of connecting the lines (Fermi statistics — a reading, the sign of the interference has no closed-form pin
+    here); pinned are the symmetry under exchange of the identical quarks and the singular limits, where one pairing
+    dominates.
 """
 import math
 from concurrent.futures import ThreadPoolExecutor
@@ -142,6 +149,78 @@ def test_charge_conjugation_and_beam_exchange(orc):
         assert abs(orc.me_qchannel("qgtTq", p) / orc.me_qchannel("QgtTQ", c) - 1) < 1e-10
         b = p[[1, 0, 2, 3, 4]]                   # beams exchanged
         assert abs(orc.me_qchannel("qgtTq", p) / orc.me_qchannel("gqtTq", b) - 1) < 1e-10
+
+
+def _perp(k):
+    k3 = k[1:] / np.linalg.norm(k[1:])
+    a = np.cross(k3, [0.0, 0.0, 1.0])
+    a /= np.linalg.norm(a)
+    return a, np.cross(k3, a)
+
+
+def test_two_lines_relabelling_symmetries(orc):
+    p = orc.rambo(31, 1, [MT, MT, 0.0, 0.0], 1500.0)[0]
+    v = orc.me_qchannel("qQtTrR", p)
+    assert v > 0 and abs(orc.me_qchannel("qQtTRr", p[[0, 1, 2, 3, 5, 4]]) / v - 1) < 1e-12
+    v = orc.me_qchannel("qrtTqr", p)
+    assert abs(orc.me_qchannel("rqtTqr", p[[1, 0, 2, 3, 4, 5]]) / v - 1) < 1e-12
+    assert abs(orc.me_qchannel("qrtTrq", p[[0, 1, 2, 3, 5, 4]]) / v - 1) < 1e-12
+    assert abs(orc.me_qchannel("QRtTQR", p[[0, 1, 3, 2, 4, 5]]) / v - 1) < 1e-10          # charge conjugation
+    v = orc.me_qchannel("qqtTqq", p)                                                        # identical quarks
+    assert abs(orc.me_qchannel("qqtTqq", p[[0, 1, 2, 3, 5, 4]]) / v - 1) < 1e-12
+    assert abs(orc.me_qchannel("qqtTqq", p[[1, 0, 2, 3, 4, 5]]) / v - 1) < 1e-12
+    assert abs(orc.me_qchannel("QQtTQQ", p[[0, 1, 3, 2, 4, 5]]) / v - 1) < 1e-10
+    # a pair of another flavour in the final state is one of the two pairings of the same-flavour process
+    assert orc.me_qchannel("qQtTqQ", p) != orc.me_qchannel("qQtTrR", p)
+
+
+def test_final_state_pair_collinear_limit_onto_the_one_jet_process(orc):
+    """q q~ -> t t~ r r~ with r || r~  ->  (2 g^2 / s_rr~) T_R (1 - 2 z (1 - z)) |M(q q~ -> t t~ g)|^2."""
+    ev = orc.rambo(32, 1, [MT, MT, 0.0], 1500.0)[0]
+    ref = orc.me_qchannel("qQtTg", ev)
+    k = ev[4]
+    a, b = _perp(k)
+    z = 0.3
+    for kt, tol in ((1e-1, 1e-3), (1e-2, 1e-4)):
+        tot = 0.0
+        for phi in (0.4, 0.4 + math.pi / 2):
+            n = math.cos(phi) * a + math.sin(phi) * b
+            p1, p2 = np.zeros(4), np.zeros(4)
+            p1[1:] = z * k[1:] + kt * n
+            p2[1:] = (1 - z) * k[1:] - kt * n
+            p1[0], p2[0] = np.linalg.norm(p1[1:]), np.linalg.norm(p2[1:])
+            Q = ev[2] + ev[3] + p1 + p2                      # beams along z that carry exactly this total
+            pa = np.array([(Q[0] + Q[3]) / 2, 0, 0, (Q[0] + Q[3]) / 2])
+            pb = np.array([(Q[0] - Q[3]) / 2, 0, 0, -(Q[0] - Q[3]) / 2])
+            v = orc.me_qchannel("qQtTrR", np.array([pa, pb, ev[2], ev[3], p1, p2]))
+            tot += v * 2 * mdot(p1, p2) / (2 * G2) / (TR * (1 - 2 * z * (1 - z)))
+        assert abs(tot / 2 / ref - 1) < tol, (kt, tot / 2 / ref)
+
+
+def test_initial_state_quark_to_gluon_limit_of_the_two_line_process(orc):
+    """q r -> t t~ q r with the final q along the incoming q: -> g^2 C_F (1 + (1-x)^2)/x / (x p_a.k) |M(g r -> t t~ r)|^2,
+    the gluon's spin correlation cancelled by two azimuths pi/2 apart."""
+    x = 0.7
+    r_out = np.array([0.0, 70.0, -90.0, 40.0])
+    r_out[0] = np.linalg.norm(r_out[1:])
+    res = {}
+    for theta in (1e-2, 1e-3):
+        tot = 0.0
+        for phi in (0.7, 0.7 + math.pi / 2):
+            E = 750.0
+            pa, pb = np.array([E, 0, 0, E]), np.array([E, 0, 0, -E])
+            k = (1 - x) * E * np.array([1, math.sin(theta) * math.cos(phi), math.sin(theta) * math.sin(phi), math.cos(theta)])
+            Q = pa + pb - k - r_out
+            M = math.sqrt(mdot(Q, Q))
+            pp = math.sqrt(M * M / 4 - MT * MT)
+            t = np.array([M / 2, pp * 0.8 * math.cos(1.1), pp * 0.8 * math.sin(1.1), pp * 0.6])
+            tb = np.array([M / 2, -t[1], -t[2], -t[3]])
+            t, tb = _boost(t, Q), _boost(tb, Q)
+            v = orc.me_qchannel("qrtTqr", np.array([pa, pb, t, tb, k, r_out]))
+            ref = orc.me_qchannel("gqtTq", np.array([x * pa, pb, t, tb, r_out]))
+            tot += v / (G2 * CF * (1 + (1 - x) ** 2) / x / (x * mdot(pa, k)) * ref)
+        res[theta] = abs(tot / 2 - 1)
+    assert res[1e-3] < 3e-3 and res[1e-3] < 0.2 * res[1e-2], res
 
 
 def test_bad_specs_are_rejected(orc):
