@@ -46,7 +46,8 @@ typedef enum {
   MG_ERR_ALIGN = -5,      /* a device pointer is not 16-byte aligned                   */
   MG_ERR_KINEMATICS = -6, /* sqrt_s <= sum of final-state masses                       */
   MG_ERR_CUDA = -7,       /* a CUDA call failed; text in mg_last_error()               */
-  MG_ERR_NO_DEVICE = -8   /* no CUDA device / bad ordinal                              */
+  MG_ERR_NO_DEVICE = -8,  /* no CUDA device / bad ordinal                              */
+  MG_ERR_TOO_LARGE = -9   /* beyond the fixed maximum of a no-allocation entry point; text in mg_last_error() */
 } mg_status_t;
 
 typedef enum { MG_FP64 = 0, MG_FP32 = 1 } mg_precision_t;
@@ -136,6 +137,20 @@ size_t mg_workspace_bytes(const mg_process_t* p, int64_t nevt);
  *     out_dev[0] = max_i, out_dev[1] = sum_i, out_dev[2] = sum_i of squares        of the products (doubles).
  * Fixed reduction tree: results are bit-reproducible.  nevt = 0 gives (-inf, 0, 0).  Asynchronous on `stream`. */
 int mg_weight_max(mg_process_t* p, void* me_dev, const double* weights_dev, int64_t nevt, double* out_dev, void* stream);
+
+/* The same primitive for callers that cannot allocate device memory (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): no handle (mg_process_create allocates), no cudaMalloc / cudaFree / allocating
+ * library call.  The first reduction stage's partial results live in a fixed 24 KiB __device__ array inside the library
+ * (every GPU that loads the library holds it until the process exits), hence the limit
+ *     nevt <= MG_NOALLOC_MAX_EVENTS = 8 388 608;   beyond it: MG_ERR_TOO_LARGE, nothing is launched.
+ * precision: mg_precision_t of me_dev's elements; runs on the CURRENT device (the first call on a device looks up the
+ * array's device address, nothing else is set up); arguments, results and reduction tree as mg_weight_max — both give
+ * bit-identical results.  All calls on one device share the scratch array: calls that overlap on the GPU (different
+ * streams, concurrently replayed graphs) race on it and must be serialised by the caller; calls on one stream are safe.
+ * Asynchronous on `stream`. */
+#define MG_NOALLOC_MAX_EVENTS 8388608LL
+int mg_weight_max_noalloc(int precision, void* me_dev, const double* weights_dev, int64_t nevt, double* out_dev,
+                          void* stream);
 
 /* Same from HOST buffers (momenta_host: layout above, me_out_host: nevt elements; pinned memory recommended): copies
  * in, runs, copies out and synchronises.  The device staging buffers belong to the handle, grow on demand and are

@@ -21,7 +21,7 @@ HEL_FILTER, HEL_ALL = 0, 1
 SYMBOLS = ["mg_params_default", "mg_process_create", "mg_process_destroy", "mg_rambo", "mg_rambo_ex", "mg_philox_raw", "mg_sigma",
            "mg_sigma_host", "mg_helicity_probe", "mg_sigma_per_helicity", "mg_good_helicities", "mg_process_info",
            "mg_momenta_bytes", "mg_set_workspace", "mg_workspace_bytes", "mg_weight_max", "mg_sigma_mixed", "mg_status_string", "mg_last_error",
-           "mg_multi_create", "mg_multi_destroy", "mg_multi_count", "mg_multi_name", "mg_multi_process", "mg_multi_sigma"]
+           "mg_weight_max_noalloc", "mg_multi_create", "mg_multi_destroy", "mg_multi_count", "mg_multi_name", "mg_multi_process", "mg_multi_sigma"]
 
 
 class MgParams(C.Structure):
@@ -75,6 +75,7 @@ def lib():
         L.mg_workspace_bytes.argtypes = [vp, i64]
         L.mg_workspace_bytes.restype = C.c_size_t
         L.mg_weight_max.argtypes = [vp, vp, vp, i64, vp, vp]
+        L.mg_weight_max_noalloc.argtypes = [C.c_int, vp, vp, i64, vp, vp]
         L.mg_sigma_mixed.argtypes = [vp, vp, i64, vp, C.c_double, vp, C.POINTER(i64), vp]
         L.mg_multi_create.argtypes = [C.c_char_p, C.POINTER(MgParams), C.POINTER(vp)]
         L.mg_multi_destroy.argtypes = [vp]
@@ -97,7 +98,7 @@ def status_string(status):
 
 def _check(rc):
     if rc != 0:
-        raise MgError(rc, lib().mg_last_error().decode() if rc == -7 else "")
+        raise MgError(rc, lib().mg_last_error().decode() if rc in (-7, -9) else "")
 
 
 def default_params(precision=FP64, helicity_mode=HEL_FILTER, device=0, **kw):
@@ -239,6 +240,24 @@ class Process:
         buf = (C.c_int32 * 256)()
         _check(lib().mg_good_helicities(self._h, buf, 256, C.byref(n)))
         return [int(buf[i]) for i in range(n.value)]
+
+
+NOALLOC_MAX_EVENTS = 8388608
+
+
+def weight_max_noalloc(me, weights, nevt=None, out=None, stream=None):
+    """mg_weight_max_noalloc: me <- weights * me in place and (max, sum, sum of squares) of the products into `out`
+    (3 doubles, caller-provided so that nothing is allocated here; created with torch.empty if None).  No handle, no
+    device allocation inside the library; nevt <= NOALLOC_MAX_EVENTS; calls on one device must not overlap."""
+    import torch
+    if nevt is None:
+        nevt = me.numel()
+    if out is None:
+        out = torch.empty(3, dtype=torch.float64, device=me.device)
+    prec = FP64 if me.dtype == torch.float64 else FP32
+    _check(lib().mg_weight_max_noalloc(prec, C.c_void_p(me.data_ptr()), C.c_void_p(weights.data_ptr()), nevt,
+                                       C.c_void_p(out.data_ptr()), _stream_ptr(stream)))
+    return out
 
 
 class MultiProcess:

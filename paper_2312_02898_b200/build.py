@@ -24,7 +24,7 @@ PEAK_LIB = os.path.join(HERE, "libmg5b200_peak.so")     # measurement helper for
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 FLAGS = ["-O3", "-std=c++17", "-lineinfo", "-rdc=true", "-Xcompiler", "-fPIC", "-I", CSRC]
-HAND = ("mg_api.cu", "mg_rambo.cu", "mg_reduce.cu")
+HAND = ("mg_api.cu", "mg_rambo.cu", "mg_reduce.cu", "mg_noalloc.cu")
 
 
 def generate(overrides=None):

@@ -24,6 +24,7 @@ static int fail(int status, const char* what) {
   snprintf(g_err, sizeof g_err, "%s", what);
   return status;
 }
+void mg_set_last_error(const char* text) { snprintf(g_err, sizeof g_err, "%s", text); }
 #define MG_CUDA(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cuda_fail(e_, #call); } while (0)
 
 struct mg_process {
@@ -594,6 +595,7 @@ const char* mg_status_string(int s) {
     case MG_ERR_KINEMATICS: return "sqrt_s not above the final-state mass threshold";
     case MG_ERR_CUDA: return "CUDA error";
     case MG_ERR_NO_DEVICE: return "no CUDA device";
+    case MG_ERR_TOO_LARGE: return "size beyond the fixed maximum of a no-allocation entry point";
     default: return "unknown status";
   }
 }

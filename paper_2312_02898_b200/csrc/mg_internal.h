@@ -24,3 +24,5 @@ cudaError_t mg_launch_mixed_flag(const float* perhel, const double* mom, long lo
                                  cudaStream_t st);
 cudaError_t mg_launch_mixed_gather(const double* mom, const int* flagged, int n, int npar, double* out, cudaStream_t st);
 cudaError_t mg_launch_mixed_scatter(const double* me64, const int* flagged, int n, double* me_out, cudaStream_t st);
+// mg_api.cu: sets the thread's mg_last_error() text (for translation units other than mg_api.cu)
+void mg_set_last_error(const char* text);

@@ -54,6 +54,10 @@ def test_status_strings_and_argument_errors_without_gpu():
     assert L.mg_multi_create(b"p p > b b~ j", C.byref(p), C.byref(h)) == -2        # nothing generated matches
     assert L.mg_multi_create(b"p p > t t~ > j", C.byref(p), C.byref(h)) == -2
     assert L.mg_multi_count(None) == 0 and L.mg_multi_sigma(None, None, 0, None, None) == -1
+    # no-allocation entry point: size beyond its fixed scratch is refused before any CUDA call
+    buf = (C.c_double * 4)()
+    assert L.mg_weight_max_noalloc(0, buf, buf, 8388608 + 1, buf, None) == -9 and b"MG_NOALLOC_MAX_EVENTS" in L.mg_last_error()
+    assert L.mg_weight_max_noalloc(0, buf, buf, -1, buf, None) == -4
     p.struct_size = 12
     assert L.mg_process_create(b"g g > t t~", C.byref(p), C.byref(h)) == -3       # MG_ERR_BAD_PARAM
     p = mg.default_params(gamma_t=1.5)
