@@ -36,7 +36,7 @@ def parse():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--workload", default="ggttgg",
-                    choices=list(workloads.CONFIGS) + ["quark_" + q for q in workloads.QUARK_SPECS],
+                    choices=list(workloads.CONFIGS) + ["quark_" + q for q in workloads.QUARK_SPECS + workloads.QUARK2_SPECS],
                     help="a BASELINE.json config, or quark_<spec>: one quark channel of p p > t t~ + jets (SURVEY 8f-3; not a "
                          "BASELINE.json config: reported for the record, no cpu_baseline leg)")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])

@@ -9,7 +9,10 @@
  * (leading order, fixed couplings: PAPER.md:141), and the quark channels of p p > t t~ + 0..2 jets that have one
  * light-quark line ("p p -> t t~ 0-2 j"; q = one massless flavour other than the top):
  *     "q q~ > t t~ [g [g]]", "q~ q > t t~ [g [g]]", "q g > t t~ q [g]", "g q > t t~ q [g]", "q~ g > t t~ q~ [g]",
- *     "g q~ > t t~ q~ [g]", "g g > t t~ q q~";   several subprocesses behind one handle: mg_multi_* below.
+ *     "g q~ > t t~ q~ [g]", "g g > t t~ q q~";
+ * and those with two light-quark lines (r: a second massless flavour; same flavour twice includes the Fermi interference):
+ *     "q q~ > t t~ r r~", "q r > t t~ q r", "q r~ > t t~ q r~", "q~ r > t t~ q~ r", "q~ r~ > t t~ q~ r~", "q q~ > t t~ q q~",
+ *     "q q > t t~ q q", "q~ q~ > t t~ q~ q~" (+ "q~ q > ...");   several subprocesses behind one handle: mg_multi_* below.
  *
  * Plain C: opaque handle, plain pointers and sizes.  Every `*_dev` pointer is DEVICE memory owned by the
  * caller (the library never frees or reallocates it); `stream` is a cudaStream_t passed as void* (NULL =
@@ -185,11 +188,14 @@ int mg_good_helicities(const mg_process_t* p, int32_t* out, int32_t capacity, in
 
 /* Several subprocesses behind one handle ("Processes with multiple subprocesses, such as
  * proton-proton collisions p p -> t t~ 0-2 j ... are being tested").  `proc` may use the multi-particle labels p (beams)
- * and j (jets) = {g, q, q~} (q: one massless quark flavour other than the top), e.g. "p p > t t~ j": it is expanded to
- * every combination, the jets as a multiset, and the combinations for which a subprocess exists are kept — the gluon
- * channels g g > t t~ (g (g)) and the 15 subprocesses with one light-quark line (q q~ > t t~ g, q g > t t~ q, ...,
- * g g > t t~ q q~).  NOT generated: the 2-jet subprocesses with two light-quark lines (q q~ > t t~ q' q'~, q q' > t t~ q q',
- * ...); mg_multi_name lists what the handle holds.  MG_ERR_BAD_PROC if nothing matches.
+ * and j (jets) = {g, q, q~, r, r~} (q, r: two distinct massless quark flavours other than the top), e.g. "p p > t t~ j":
+ * it is expanded to every combination and the combinations for which a subprocess was generated are kept — the gluon
+ * channels g g > t t~ (g (g)), the 15 subprocesses with one light-quark line (q q~ > t t~ g, q g > t t~ q, ...,
+ * g g > t t~ q q~) and the 10 two-jet subprocesses with two light-quark lines (q q~ > t t~ r r~, q r > t t~ q r,
+ * q r~ > t t~ q r~, q~ r > t t~ q~ r, q~ r~ > t t~ q~ r~, q q~ > t t~ q q~, q q > t t~ q q, q~ q~ > t t~ q~ q~, and the two
+ * with q~ q beams).  Matrix elements do not depend on which flavours q and r are; one generated function per distinct
+ * particle order (e.g. "r q > t t~ r q" is "q r > t t~ q r" with the momenta of the beams and of the jets exchanged and is
+ * not generated separately).  mg_multi_name lists what the handle holds.  MG_ERR_BAD_PROC if nothing matches.
  * mg_multi_sigma: |M|^2 of every subprocess on the SAME nevt momenta (all share npar and the momenta layout);
  * me_out_dev[isub * nevt + ievt], element type of the precision.  PDFs and the sum over subprocesses stay with the caller
  * (host side).  mg_multi_process returns the borrowed single-subprocess handle (owned by the multi handle)

@@ -30,7 +30,8 @@
  * initial-state collinear limits q -> q g and g -> q q~ onto the closed form (every 1-jet process) and of
  * q q~ -> t t~ g g onto q q~ -> t t~ g, C- and beam-exchange symmetries.  The other 2-jet crossings with one light line
  * (q g -> t t~ q g, g g -> t t~ q q~, ...) run the same code with other external spinors; their own pins are the Ward
- * identities.  Two light lines: see the test file's header.
+ * identities.  Two light lines: see the test file's header; the SIGN of the interference between the two pairings of the
+ * same-flavour processes is a reading with no pin of its own ("parity unpinned" for that term).
  */
 #include "oracle_internal.h"
 

@@ -33,6 +33,7 @@ def generate(overrides=None):
     import json
     from .gen.emit import emit_eemumu, emit_ggttng
     from .gen.quark import SPECS, emit_quark
+    from .gen.quark2 import SPECS as SPECS2, emit_quark2
     os.makedirs(GEN, exist_ok=True)
     infos, paths = [], []
     jobs = [emit_eemumu()]
@@ -42,6 +43,8 @@ def generate(overrides=None):
         jobs.append(emit_ggttng(n, **kw))
     for spec in SPECS:                       # quark channels of p p -> t t~ + 0..2 jets
         jobs.append(emit_quark(spec))
+    for spec in SPECS2:                      # ... with two light-quark lines (2 jets, no gluon)
+        jobs.append(emit_quark2(spec))
     keep = set()
     for files, info in jobs:
         for fname, src in files:

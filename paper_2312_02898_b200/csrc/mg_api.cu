@@ -497,7 +497,7 @@ int mg_process_info(const mg_process_t* p, mg_info_t* o) {
 
 // ---------------------------------------------------------------------------------------------------------------
 // Several subprocesses behind one handle ("processes with multiple subprocesses, such as p p -> t t~ 0-2 j").
-// `p` (beams) and `j` (jets) stand for {g, q, q~}; the string is expanded to every combination, jets as a multiset, and
+// `p` (beams) and `j` (jets) stand for {g, q, q~, r, r~}; the string is expanded to every combination, jets as a multiset, and
 // the combinations for which a subprocess was generated are kept (quark number is conserved by construction: the others
 // do not exist).  All subprocesses share npar, hence one momenta buffer.
 // ---------------------------------------------------------------------------------------------------------------
@@ -526,22 +526,23 @@ int mg_multi_create(const char* proc, const mg_params_t* params, mg_multi_t** ou
     }
   }
   if (ini.size() != 2 || fin.size() < 2 || fin.size() > 6) return MG_ERR_BAD_PROC;
-  static const char* const parton[3] = {"g", "q", "q~"};
+  static const char* const parton[5] = {"g", "q", "q~", "r", "r~"};     // q, r: two distinct massless flavours
+  constexpr int NP = 5;
   std::vector<int> jets;                           // positions of the j's in the final state
   for (size_t i = 0; i < fin.size(); ++i) if (fin[i] == "j") jets.push_back((int)i);
   const int nj = (int)jets.size();
   int ncomb = 1;
-  for (int i = 0; i < nj; ++i) ncomb *= 3;
+  for (int i = 0; i < nj; ++i) ncomb *= NP;
   mg_multi* m = new mg_multi();
   int rc = MG_OK;
-  for (int a = 0; a < 3 && rc == MG_OK; ++a) {
+  for (int a = 0; a < NP && rc == MG_OK; ++a) {
     if (ini[0] != "p" && a > 0) break;
-    for (int b = 0; b < 3 && rc == MG_OK; ++b) {
+    for (int b = 0; b < NP && rc == MG_OK; ++b) {
       if (ini[1] != "p" && b > 0) break;
       for (int c = 0; c < ncomb && rc == MG_OK; ++c) {
         std::vector<std::string> f = fin;
         int r = c;
-        for (int i = 0; i < nj; ++i) { f[jets[i]] = parton[r % 3]; r /= 3; }
+        for (int i = 0; i < nj; ++i) { f[jets[i]] = parton[r % NP]; r /= NP; }
         std::string name = std::string(ini[0] == "p" ? parton[a] : ini[0].c_str()) + " " +
                            (ini[1] == "p" ? parton[b] : ini[1].c_str()) + " >";
         for (const std::string& t : f) name += " " + t;

@@ -81,3 +81,52 @@ def test_every_subprocess_is_emitted_with_its_averaging_factor():
     files, info = Q.emit_quark("qgtTqg")
     assert info["ndiagrams"] == 36 and info["ncol"] == 12 and info["proc"] == "q g > t t~ q g"
     assert "cur_pair" in files[0][1] and "mg_desc_qgttxqg" in files[0][1]
+
+
+# ------------------------------------------------------------------------------------------- two light-quark lines
+def test_two_line_term_colours_equal_the_explicit_gell_mann_tensors():
+    """Each of the seven terms: sum over the pseudo-gluon colours of the T-strings on the three open lines (numpy, explicit
+    Gell-Mann matrices) against the generator's Fierz-reduced combination of Kronecker deltas."""
+    from paper_2312_02898_b200.gen import quark2 as Q2
+    T = gell_mann()
+    rows, cols = ("t", "e0", "e1"), ("T", "s0", "s1")
+    eye = np.eye(3)
+    for kind, strings in Q2.terms():
+        want = np.zeros((3,) * 6, dtype=complex)           # indices: t, T, e0, s0, e1, s1
+        for sign, top, l0, l1 in strings:
+            for x0 in range(8):
+                for x1 in range(8):
+                    lab = {"P0": T[x0], "P1": T[x1]}
+
+                    def mat(s):
+                        m = eye.astype(complex)
+                        for a in s:
+                            m = m @ lab[a]
+                        return m
+
+                    want += sign * np.einsum("ab,cd,ef->abcdef", mat(top), mat(l0), mat(l1))
+        got = np.zeros((3,) * 6, dtype=complex)
+        pos = {"t": 0, "T": 1, "e0": 2, "s0": 3, "e1": 4, "s1": 5}
+        for flow, coef in Q2.term_colour(strings, rows, cols, rows).items():
+            letters = "abcdef"
+            ops = []
+            for r, c in zip(rows, flow):
+                ops.append(letters[pos[r]] + letters[pos[c]])
+            got += float(coef) * np.einsum("%s,%s,%s->abcdef" % tuple(ops), eye, eye, eye)
+        assert np.abs(got - want).max() < 1e-12, kind
+
+
+def test_two_line_flow_matrix_and_processes():
+    from paper_2312_02898_b200.gen import quark2 as Q2
+    rows = ("t", "e0", "e1")
+    from itertools import permutations
+    flows = list(permutations(("T", "s0", "s1")))
+    cf = np.array(Q2.flow_matrix(flows, rows))
+    assert cf.shape == (6, 6) and np.all(np.diag(cf) == 27) and set(cf.ravel()) == {3, 9, 27}
+    assert np.array_equal(cf, cf.T) and np.linalg.matrix_rank(cf) == 6
+    assert Q2.QProcess2("qQtTrR").denominator == 36 and Q2.QProcess2("qqtTqq").denominator == 72
+    assert len(Q2.QProcess2("qQtTqQ").pairings) == 2 and len(Q2.QProcess2("qrtTqr").pairings) == 1
+    files, info = Q2.emit_quark2("qQtTqQ")
+    assert info["ndiagrams"] == 14 and info["ncol"] == 6 and info["proc"] == "q q~ > t t~ q q~"
+    files, info = Q2.emit_quark2("qRtTqR")
+    assert info["ndiagrams"] == 7 and "mg_desc_qrxttxqrx" in files[0][1]

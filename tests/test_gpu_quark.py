@@ -12,6 +12,7 @@ pytestmark = pytest.mark.gpu
 
 # events per subprocess: the oracle costs ~2 ms (0 jets), 0.1 s (1 jet), 5 s (2 jets) per event and core
 NEVT = {4: 4133, 5: 1029, 6: 37}
+NEVT2 = 261                      # two light lines, no gluon: 0.25 - 0.5 s per event
 
 
 @pytest.fixture(scope="module")
@@ -23,11 +24,11 @@ def mg():
     return m
 
 
-@pytest.mark.parametrize("spec", workloads.QUARK_SPECS)
+@pytest.mark.parametrize("spec", workloads.QUARK_SPECS + workloads.QUARK2_SPECS)
 def test_quark_channel_fp64_parity(mg, oracle, oracle_ld, spec):
     import torch
     cfg = workloads.QUARK_CHANNELS[spec]
-    nevt = NEVT[len(spec)]
+    nevt = NEVT2 if spec in workloads.QUARK2_SPECS else NEVT[len(spec)]
     ref = None
     for mode in (mg.HEL_ALL, mg.HEL_FILTER):
         proc = mg.Process(cfg["proc"], helicity_mode=mode)
@@ -48,7 +49,7 @@ def test_quark_channel_fp64_parity(mg, oracle, oracle_ld, spec):
         proc.close()
 
 
-@pytest.mark.parametrize("spec", ["qQtTg", "gQtTQ", "qgtTqg"])
+@pytest.mark.parametrize("spec", ["qQtTg", "gQtTQ", "qgtTqg", "qrtTqr", "qQtTqQ"])
 def test_quark_channel_per_helicity_and_filter(mg, oracle, spec):
     """Per-helicity |M_h|^2 against the oracle's, and the helicity bookkeeping: chirality conservation along the massless
     line halves the good helicities, the helicity-flip symmetry halves the evaluated ones again."""
@@ -60,8 +61,14 @@ def test_quark_channel_per_helicity_and_filter(mg, oracle, spec):
     proc.helicity_probe(mom, nevt)
     info = proc.info
     assert info.nhel == 1 << len(spec)
-    assert info.ngoodhel == info.nhel // 2
-    assert info.nhel_evaluated == info.nhel // 4
+    # chirality along every massless line: each line halves the non-vanishing helicities (same flavour twice: either
+    # pairing may conserve it, 6 of the 16 light-quark helicity combinations survive)
+    nlines = sum(c in "qQrR" for c in spec) // 2
+    frac = {1: 2, 2: 4}[nlines] if set(spec) & set("rR") or nlines == 1 else None
+    if frac:
+        assert info.ngoodhel == info.nhel // frac and info.nhel_evaluated == info.nhel // (2 * frac)
+    else:
+        assert info.ngoodhel == info.nhel * 6 // 16 and info.nhel_evaluated == info.ngoodhel // 2
     ph = proc.sigma_per_helicity(mom, nevt)
     torch.cuda.synchronize()
     ph = ph.cpu().numpy()
@@ -89,7 +96,7 @@ def test_quark_channel_fp32(mg, oracle, spec):
     p32.close()
 
 
-@pytest.mark.parametrize("proc,nsub,nevt", [("p p > t t~", 3, 512), ("p p > t t~ j", 7, 256), ("p p > t t~ j j", 8, 16)])
+@pytest.mark.parametrize("proc,nsub,nevt", [("p p > t t~", 3, 512), ("p p > t t~ j", 7, 256), ("p p > t t~ j j", 18, 16)])
 def test_multi_subprocess_handle(mg, oracle, proc, nsub, nevt):
     """Several subprocesses behind one handle, evaluated on the SAME momenta (what a p p -> t t~ + jets event needs before
     the PDFs weight them): every row against the oracle of its subprocess."""

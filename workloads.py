@@ -28,14 +28,17 @@ PROC_TO_NAME = {v["proc"]: k for k, v in CONFIGS.items()}
 # Quark channels of p p -> t t~ + 0..2 jets with one light-quark line.  Key: one character
 # per particle in process order ('q' light quark, 'Q' light antiquark, 'g' gluon, 'tT' = t t~); not BASELINE.json
 # configs: parity-test workloads only (sqrt(s) and the RAMBO recipe as for the gluon channels).
-_QNAMES = {"q": "q", "Q": "q~", "g": "g", "t": "t", "T": "t~"}
+_QNAMES = {"q": "q", "Q": "q~", "r": "r", "R": "r~", "g": "g", "t": "t", "T": "t~"}
 QUARK_SPECS = ("qQtT", "QqtT",
                "qQtTg", "QqtTg", "qgtTq", "gqtTq", "QgtTQ", "gQtTQ",
                "qQtTgg", "QqtTgg", "qgtTqg", "gqtTqg", "QgtTQg", "gQtTQg", "ggtTqQ")
+# two light-quark lines ('r' / 'R': quark / antiquark of a second light flavour), no gluon
+QUARK2_SPECS = ("qQtTrR", "QqtTrR", "qrtTqr", "qRtTqR", "QrtTQr", "QRtTQR",
+                "qQtTqQ", "QqtTqQ", "qqtTqq", "QQtTQQ")
 QUARK_CHANNELS = {
     spec: dict(proc=" ".join(_QNAMES[c] for c in spec[:2]) + " > " + " ".join(_QNAMES[c] for c in spec[2:]),
                sqrt_s=1500.0, seed=20 + i, masses_final=[MT, MT] + [0.0] * (len(spec) - 4))
-    for i, spec in enumerate(QUARK_SPECS)
+    for i, spec in enumerate(QUARK_SPECS + QUARK2_SPECS)
 }
 
 GOLDEN_DIR = os.path.join(os.path.dirname(os.path.abspath(__file__)), "tests", "golden")
