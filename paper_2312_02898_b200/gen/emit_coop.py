@@ -86,18 +86,34 @@ def _pack(groups, limit):
 def families(n, max_phase, min_class=6):
     """[dict(kind, size, members=[pi, ...], bodies=[[term, ...], ...])]: the canonical class of every family, cut into
     bodies, and the relabellings pi (tuples: canonical gluon i -> actual gluon pi[i]) of its members.  Classes with
-    fewer than `min_class` terms are not worth a visit per member: their terms are emitted as they are, together, in a
+    fewer than `min_class` terms are not worth a visit per member: small classes over the same gluon subsets (same
+    relabellings) are merged into one family if that makes them big enough, the rest is emitted as it is, together, in a
     last family with the identity as its only member."""
     classes = {}
     for term in topo.diagram_terms(n):
         kind, S = family_key(term, n)
         classes.setdefault((kind, len(S)), {}).setdefault(S, []).append(term)
-    out, misc = [], []
+    out, misc, small = [], [], {}
+    normal = []
     for (kind, size), cls in sorted(classes.items()):
         sizes = {len(v) for v in cls.values()}
-        if not (len(sizes) == 1 and len(cls) == comb(n, size)) or min(sizes) < min_class:
-            misc += [t for S in sorted(cls) for t in cls[S]]      # key not equivariant (ties), or class too small
-            continue
+        if not (len(sizes) == 1 and len(cls) == comb(n, size)):
+            misc += [t for S in sorted(cls) for t in cls[S]]      # key not equivariant (ties)
+        elif min(sizes) < min_class:
+            small.setdefault(size, []).append((kind, cls))        # class too small for a visit of its own
+        else:
+            normal.append((kind, size, cls))
+    # small classes over the same gluon subsets share their relabellings: together they may be worth a visit per member
+    for size, lst in sorted(small.items()):
+        merged = {}
+        for _, cls in lst:
+            for S, ts in cls.items():
+                merged.setdefault(S, []).extend(ts)
+        if len(lst) > 1 and len(merged[min(merged)]) >= min_class:
+            normal.append(("+".join(k for k, _ in lst), size, merged))
+        else:
+            misc += [t for _, cls in lst for S in sorted(cls) for t in cls[S]]
+    for kind, size, cls in normal:
         S0 = min(cls)
         rest0 = [i for i in range(n) if i not in S0]
         members = []
