@@ -588,10 +588,10 @@ def _main_unit(E, n, ns, hdr, cfi, cfden, fams, bodies, bmeta, invmap, flowmap, 
             % (bi, fams[fi]["kind"], fams[fi]["size"], len(b.plan.terms), nm_, nm_, v0, foff_of[fi], bi))
     w(KERNEL % dict(calls="".join(calls), minb=cfg.get("ctas_per_sm", 256 // BLK),
                     colour=("T meh;\n    if constexpr (sizeof(T) == 8) {\n"
-                            "      colour_dmma_cta<NCOL, BLK>(cf_dense, (const double*)jamp_cta, reinterpret_cast<double*>(smem_raw), (double*)s_meh);\n"
+                            "      colour_dmma_cta<NCOL, BLK>(cf_dense, (const double*)jamp_cta, reinterpret_cast<double*>(smem_raw + SINV_BYTES), (double*)s_meh);\n"
                             "      meh = s_meh[tid];\n    } else meh = colour_reg<T>(jamp);" if dmma else
                             "T meh = colour_reg<T>(jamp);"),
-                    coloursm=(2 * ncol * 34 + (BLK // 32) * 32) * 8 if dmma else 0))
+                    coloursm=((2 * ncol * 34 + (BLK // 32) * 32) * 8 + ((BLK // hdr["nlane"]) * ninvp * 8 + 15) // 16 * 16) if dmma else 0))
     w(LAUNCH % dict(cfden=cfden, denom=denom, minb=cfg.get("ctas_per_sm", 256 // BLK), l2win=1 if cfg.get("l2_window") else 0,
                     run32=("  return run<float>(mom, (float*)me_out, nevt, (const float*)lane_w, ntb, tb_first, (float*)perhel_out, par, ws, ws_bytes, st);"
                            if fp32 else "  return -1;")))
@@ -634,23 +634,20 @@ sigma_kernel(long long nevt, int ntb, int tb_first, const T* __restrict__ lane_w
   const unsigned sj = sfm0 + 2 * NFLOWS * 4 + ((NTABS & 1) ? 4 : 0) + tid * SZ;
   const unsigned sinvp = sinvp0 + slot * NINVS * SZ;
   const T* __restrict__ asgn = amp_sign_of((T*)nullptr);
-  T* __restrict__ sinv_g = reinterpret_cast<T*>(smem_raw);
+  constexpr unsigned SINV_BYTES = (SLOTS * NINVP * SZ + 15u) / 16u * 16u;      // the colour sum's tile staging starts behind it
   T* __restrict__ jamp_cta = scratch + (size_t)blockIdx.x * (2 * NCOL * BLK + SLOTS * NTABF);
   T* __restrict__ jamp = jamp_cta + tid;
   T* __restrict__ gtab = jamp_cta + 2 * NCOL * BLK;            // event-wide helicity tables of the CTA's slots
   const long long nslot = nevt * ntb;
+  prefetch_invariants<T>(invbuf, sinv0, (long long)blockIdx.x * SLOTS, nslot, nevt, ntb, NINVP, SLOTS);
   for (long long g0 = (long long)blockIdx.x * SLOTS; g0 < nslot; g0 += (long long)gridDim.x * SLOTS) {
     const long long gs = g0 + slot;
     const bool slot_live = gs < nslot;
     const long long ievt = slot_live ? (ntb == 2 ? gs >> 1 : gs) : nevt - 1;
     const int tb = ntb == 2 ? (int)(gs & 1) : tb_first;
-    __syncthreads();                       // previous iteration's shared memory is dead
+    visit_drain();                         // this group's invariants (prefetched) have landed ..
+    __syncthreads();                       // .. for every thread, and the previous iteration's shared memory is dead
     if (lane == 0) s_tbit[slot] = tb;
-    for (int i = tid; i < SLOTS * NINVP; i += BLK) {
-      const int s = i / NINVP, k = i - s * NINVP;
-      const long long e = (g0 + s) < nslot ? (ntb == 2 ? (g0 + s) >> 1 : (g0 + s)) : nevt - 1;
-      sinv_g[i] = __ldg(invbuf + e * NINVP + k);
-    }
 #pragma unroll 8
     for (int q = 0; q < 2 * NCOL; ++q) jamp[q * BLK] = T(0);      // the bodies only ever add (L2 reductions)
     // full helicity index: bit (NPAR-1-i) <=> particle i; the top quark (particle 2) sits at bit TPOS
@@ -662,6 +659,8 @@ sigma_kernel(long long nevt, int ntb, int tb_first, const T* __restrict__ lane_w
     visit_prologue<T, SLOTS>(visit_desc, tab_map, gtab, asgn, flow_map, smap0, stab0, ssgn0, sfm0, NTABS, NTABF, NAMPS, NFLOWS);
 %(calls)s
     visit_drain();
+    // nothing reads the invariant block after the last visit: the next group's invariants travel during the colour sum
+    prefetch_invariants<T>(invbuf, sinv0, g0 + (long long)gridDim.x * SLOTS, nslot, nevt, ntb, NINVP, SLOTS);
     __threadfence();                       // the JAMP reductions are performed at L2 before anyone reads them back
     __syncthreads();
     %(colour)s
