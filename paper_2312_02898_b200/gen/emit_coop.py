@@ -648,8 +648,12 @@ sigma_kernel(long long nevt, int ntb, int tb_first, const T* __restrict__ lane_w
     visit_drain();                         // this group's invariants (prefetched) have landed ..
     __syncthreads();                       // .. for every thread, and the previous iteration's shared memory is dead
     if (lane == 0) s_tbit[slot] = tb;
+    {   // the bodies only ever add (L2 reductions): zero the CTA's JAMPs, two columns per store
+      struct __align__(2 * sizeof(T)) T2 { T x, y; };
+      T2* __restrict__ z = reinterpret_cast<T2*>(jamp_cta) + tid;        // 2 NCOL BLK values = NCOL BLK pairs
 #pragma unroll 8
-    for (int q = 0; q < 2 * NCOL; ++q) jamp[q * BLK] = T(0);      // the bodies only ever add (L2 reductions)
+      for (int q = 0; q < NCOL; ++q) z[q * BLK] = T2{T(0), T(0)};
+    }
     // full helicity index: bit (NPAR-1-i) <=> particle i; the top quark (particle 2) sits at bit TPOS
     const int h = ((lane >> TPOS) << (TPOS + 1)) | (tb << TPOS) | (lane & ((1 << TPOS) - 1));
     const T wgt = lane_w[tb * NLANE + lane];
