@@ -313,6 +313,16 @@ def shard(nevt_per_gpu, rank, world_size=1):
     return rank * nevt_per_gpu, nevt_per_gpu
 
 
+def allreduce_weight_stats(out3, group=None):
+    """Combines the (max, sum, sum of squares) of mg_weight_max over the ranks that sharded the event stream (SURVEY.md §8e:
+    the only exchange a consumer of PAPER.md:101 needs: one all-reduce of three doubles per batch; the data path itself
+    has no collective).  In place on `out3` (CUDA tensor with NCCL, CPU tensor with gloo); returns it."""
+    import torch.distributed as dist
+    dist.all_reduce(out3[0:1], op=dist.ReduceOp.MAX, group=group)
+    dist.all_reduce(out3[1:3], op=dist.ReduceOp.SUM, group=group)
+    return out3
+
+
 def pages_to_events(momenta, nevt, npar):
     """AoSoA pages [page][ipar][32][4] -> plain [nevt][npar][4] (layout shuffle only; torch or numpy)."""
     pages = (nevt + NEPP - 1) // NEPP

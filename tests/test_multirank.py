@@ -31,6 +31,13 @@ def _worker(rank, world, port, nevt, out):
     mom = O.load(False).rambo(cfg["seed"], n, cfg["masses_final"], cfg["sqrt_s"], first_event=first)
     gathered = [torch.zeros(mom.shape, dtype=torch.float64) for _ in range(world)]
     dist.all_gather(gathered, torch.from_numpy(mom))           # test-only exchange: the data path has none
+    # batch-unweighting statistics of the shards: max / sum / sum of squares combine with one all-reduce
+    orc = O.load(False)
+    me = orc.me_batch(cfg["proc"], mom)
+    prod, st = orc.weight_max(me, np.full(n, 2.0))
+    st = mg.allreduce_weight_stats(torch.from_numpy(st.copy()))
+    if rank == 0:
+        np.save(out + ".stats", st.numpy())
     t = torch.tensor([0.5 + rank], dtype=torch.float64)        # per-rank timing -> max over ranks, as bench.py does
     dist.all_reduce(t, op=dist.ReduceOp.MAX)
     dist.barrier()
@@ -52,6 +59,10 @@ def test_two_ranks_shard_the_event_stream(tmp_path):
     whole = O.load(False).rambo(cfg["seed"], world * nevt, cfg["masses_final"], cfg["sqrt_s"])
     assert np.array_equal(np.load(out), whole)
     assert float(open(out + ".t").read()) == 1.5
+    orc = O.load(False)
+    prod = 2.0 * orc.me_batch(cfg["proc"], whole)
+    st = np.load(out + ".stats.npy")
+    assert st[0] == prod.max() and abs(st[1] / prod.sum() - 1) < 1e-13 and abs(st[2] / (prod * prod).sum() - 1) < 1e-13
 
 
 def test_shard_arguments():
