@@ -121,8 +121,8 @@ int mg_philox_raw(mg_process_t* p, uint64_t seed, int64_t first_event, int64_t n
  * (mg_set_workspace).  One handle serves one stream at a time: the workspace and the helicity lists belong to the
  * handle, so calls on the same handle must be ordered by the caller (distinct handles are independent).
  * Device-state side effect (g g > t t~ g g g only, scratch 108 MB): for the duration of its launches the call puts an
- * L2 access-policy window (scratch persisting, everything else streaming) on `stream` and raises the device limit
- * cudaLimitPersistingL2CacheSize to min(scratch, device maximum); the window is removed from the stream before the call
+ * L2 access-policy window (the JAMP part of the scratch persisting) on `stream` and raises the device limit
+ * cudaLimitPersistingL2CacheSize to min(73 MB, device maximum); the window is removed from the stream before the call
  * returns, the limit stays, mg_process_destroy resets the persisting lines. */
 int mg_sigma(mg_process_t* p, const void* momenta_dev, int64_t nevt, void* me_out_dev, void* stream);
 

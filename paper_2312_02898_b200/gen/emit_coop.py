@@ -619,7 +619,7 @@ KERNEL = """
 template <class T>
 __global__ void __launch_bounds__(BLK, %(minb)d)
 sigma_kernel(long long nevt, int ntb, int tb_first, const T* __restrict__ lane_w, const T* __restrict__ invbuf,
-             T* __restrict__ scratch, T* __restrict__ me_out, T* __restrict__ perhel_out,
+             T* __restrict__ scratch, T* __restrict__ gtab_all, T* __restrict__ me_out, T* __restrict__ perhel_out,
              long long perhel_stride, T norm) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   __shared__ int s_tbit[SLOTS];
@@ -635,9 +635,11 @@ sigma_kernel(long long nevt, int ntb, int tb_first, const T* __restrict__ lane_w
   const unsigned sinvp = sinvp0 + slot * NINVS * SZ;
   const T* __restrict__ asgn = amp_sign_of((T*)nullptr);
   constexpr unsigned SINV_BYTES = (SLOTS * NINVP * SZ + 15u) / 16u * 16u;      // the colour sum's tile staging starts behind it
-  T* __restrict__ jamp_cta = scratch + (size_t)blockIdx.x * (2 * NCOL * BLK + SLOTS * NTABF);
+  // scratch = [JAMPs of every resident CTA][event-wide helicity tables of every resident CTA]: the JAMP part is what the
+  // launcher's persisting L2 window covers
+  T* __restrict__ jamp_cta = scratch + (size_t)blockIdx.x * (2 * NCOL * BLK);
   T* __restrict__ jamp = jamp_cta + tid;
-  T* __restrict__ gtab = jamp_cta + 2 * NCOL * BLK;            // event-wide helicity tables of the CTA's slots
+  T* __restrict__ gtab = gtab_all + (size_t)blockIdx.x * (SLOTS * NTABF);      // event-wide helicity tables of the CTA's slots
   const long long nslot = nevt * ntb;
   prefetch_invariants<T>(invbuf, sinv0, (long long)blockIdx.x * SLOTS, nslot, nevt, ntb, NINVP, SLOTS);
   for (long long g0 = (long long)blockIdx.x * SLOTS; g0 < nslot; g0 += (long long)gridDim.x * SLOTS) {
@@ -710,19 +712,20 @@ static int run(const double* mom, T* me_out, long long nevt, const T* lane_w, in
   if (E > nevt) E = (nevt + 31) / 32 * 32;
   else { const long long nt = (nevt + E - 1) / E; E = ((nevt + nt - 1) / nt + 31) / 32 * 32; }   // equal tiles
   int nlaunch = 0;
-  // The CTA-private scratch is the kernel's working set: when it is a large part of the L2 (gg -> t t~ g g g: 108 MB of
-  // 126 MB) dirty JAMP lines are evicted and fetched again all the time (measured: 395 GB of DRAM writes per call).  An access
-  // policy window makes the scratch persisting up to the device's limit and everything else streaming (71 GB, -3.7 %% time).
-  const bool l2win = %(l2win)d && scratch_bytes > ((size_t)32 << 20);
+  // The CTA-private JAMPs are the kernel's read-modify-write working set (gg -> t t~ g g g: 73 MB, next to 35 MB of tables, in
+  // a 126 MB L2): without help dirty JAMP lines are evicted and fetched again all the time (measured: 395 GB of DRAM writes
+  // per call).  An access-policy window makes the JAMP part of the scratch persisting, up to the device's limit.
+  const size_t jamp_bytes = (size_t)ncta_max * 2 * NCOL * BLK * sizeof(T);
+  const bool l2win = %(l2win)d && jamp_bytes > ((size_t)32 << 20);
   if (l2win) {
     int maxp = 0, maxw = 0;
     cudaDeviceGetAttribute(&maxp, cudaDevAttrMaxPersistingL2CacheSize, dev);
     cudaDeviceGetAttribute(&maxw, cudaDevAttrMaxAccessPolicyWindowSize, dev);
     if (maxp > 0 && maxw > 0) {
-      const size_t setaside = scratch_bytes < (size_t)maxp ? scratch_bytes : (size_t)maxp;
+      const size_t setaside = jamp_bytes < (size_t)maxp ? jamp_bytes : (size_t)maxp;
       cudaStreamAttrValue av;
       av.accessPolicyWindow.base_ptr = (void*)scratch;
-      av.accessPolicyWindow.num_bytes = scratch_bytes < (size_t)maxw ? scratch_bytes : (size_t)maxw;
+      av.accessPolicyWindow.num_bytes = jamp_bytes < (size_t)maxw ? jamp_bytes : (size_t)maxw;
       const double ratio = (double)setaside / (double)av.accessPolicyWindow.num_bytes;
       av.accessPolicyWindow.hitRatio = ratio < 1.0 ? (float)ratio : 1.f;
       av.accessPolicyWindow.hitProp = cudaAccessPropertyPersisting;
@@ -736,7 +739,7 @@ static int run(const double* mom, T* me_out, long long nevt, const T* lane_w, in
     invariants_kernel<T><<<(unsigned)((ne + 127) / 128), 128, 0, st>>>(mom + e0 * NPAR * 4, ne, inv, par[1]);
     const long long nslot = ne * ntb, ngroup = (nslot + SLOTS - 1) / SLOTS;
     const unsigned grid = (unsigned)(ngroup < ncta_max ? ngroup : ncta_max);
-    kern<<<grid, BLK, smem, st>>>(ne, ntb, tb_first, lane_w, inv, scratch, me_out + e0,
+    kern<<<grid, BLK, smem, st>>>(ne, ntb, tb_first, lane_w, inv, scratch, scratch + (size_t)ncta_max * 2 * NCOL * BLK, me_out + e0,
                                   perhel_out ? perhel_out + e0 : (T*)nullptr, nevt, T(norm));
     nlaunch += 2;
   }
