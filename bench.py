@@ -65,15 +65,25 @@ def oracle_time(name, cfg, nsample, repeats=1):
     """Times the oracle as it stands (double build, OpenMP over events) on `nsample` events of the workload."""
     from oracle import oracle as O
     orc = O.load(False)
+    cores = host_cores()
     mom = orc.rambo(cfg["seed"], nsample, cfg["masses_final"], cfg["sqrt_s"])
     best = None
     for _ in range(repeats):
         t0 = time.perf_counter()
-        me = orc.me_batch(cfg["proc"], mom)
+        me = orc.me_batch(cfg["proc"], mom, nthreads=cores)
         dt = time.perf_counter() - t0
         best = dt if best is None else min(best, dt)
     assert (me > 0).all()
-    return nsample / best, best, orc.num_threads()
+    return nsample / best, best, cores
+
+
+def host_cores():
+    """Threads the oracle legs run on: the cores this process may use (torchrun exports OMP_NUM_THREADS=1 for N > 1, which
+    would otherwise make the oracle single-threaded)."""
+    try:
+        return max(1, len(os.sched_getaffinity(0)))
+    except AttributeError:
+        return max(1, os.cpu_count() or 1)
 
 
 def run_reference(args, name, cfg):
@@ -84,15 +94,15 @@ def run_reference(args, name, cfg):
     from oracle import oracle as O
     orc = O.load(False)
     mom = orc.rambo(cfg["seed"], nsample, cfg["masses_final"], cfg["sqrt_s"])
+    cores = host_cores()
     for _ in range(min(args.warmup, 1)):
-        orc.me_batch(cfg["proc"], mom[: max(8, nsample // 8)])
+        orc.me_batch(cfg["proc"], mom[: max(8, nsample // 8)], nthreads=cores)
     t0 = time.perf_counter()
     for _ in range(args.steps):
         mom = orc.rambo(cfg["seed"], nsample, cfg["masses_final"], cfg["sqrt_s"])
-        orc.me_batch(cfg["proc"], mom)
+        orc.me_batch(cfg["proc"], mom, nthreads=cores)
     dt = time.perf_counter() - t0
     val = nsample * args.steps / dt
-    cores = orc.num_threads()
     sample = "%d events per step (prefix of the workload's seeded RAMBO batch), oracle RAMBO + |M|^2" % nsample
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
@@ -370,7 +380,7 @@ def main():
     line.update(res)
     if also:
         line["also"] = also
-    if not args.no_cpu_baseline:
+    if not args.no_cpu_baseline and world == 1:                 # reported at N = 1 only
         ns = ORACLE_SAMPLE[name]
         v, dt, cores = oracle_time(name, cfg, ns)
         line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "seconds": dt,
