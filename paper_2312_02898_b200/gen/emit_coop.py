@@ -34,9 +34,10 @@ BLK = 256      # default threads per CTA (cfg["block"])
 # come from the per-visit helicity tables) and the shared-memory budget, per multiplicity
 # (measured on B200: gg -> tt~gg 37.9 ms with (2, 1) tables and 40-term bodies against 40.6 ms with (3, 2)
 # and 24; gg -> tt~ggg with (3, 2) and 16-term bodies: 424 ms against 500 / 562 ms with 32 / 48 at that stage; l2_window: the
-# scratch as a persisting L2 window, 387 -> 373 ms)
+# scratch as a persisting L2 window, 387 -> 373 ms; gather16: 16-byte copies of groups of four table operands, 366 -> 355 ms,
+# but 37.7 -> 38.3 ms at n = 4)
 TUNED = {4: dict(max_phase=40, gtab=2, qtab=1, smem_kb=110, block=128, sync_every=0),
-         5: dict(max_phase=16, gtab=3, qtab=2, smem_kb=110, block=128, sync_every=0, min_class=5, l2_window=True)}
+         5: dict(max_phase=16, gtab=3, qtab=2, smem_kb=110, block=128, sync_every=0, min_class=5, l2_window=True, gather16=True)}
 INV_SIZE = {"sg": 1, "pm": 4, "tl": 5, "tr": 5, "eg": 5, "ub": 16, "vv": 16}
 _ORDER = {"s": 0, "p": 1, "t": 2, "e": 3, "u": 4, "v": 5}
 
@@ -337,13 +338,16 @@ def emit_coop(n, fp32=True, acc_max=24, **over):
     ninvs = max(1, max(b.ninv for _, b in bodies))
     assert ninvs <= BLK, "visit_gather copies one helicity-independent operand per thread"
     ninvs += ninvs & 1
-    ntabs = max(b.ntab for _, b in bodies)
+    ntabs = (max(b.ntab for _, b in bodies) + 3) // 4 * 4        # 16-byte aligned slot stride in both precisions
     namps = max(b.plan.namps for _, b in bodies)
     assert namps <= BLK
+    namps += namps & 1
     nflows = max(len(b.flows) for _, b in bodies)
     nflows += nflows & 1
     assert nflows <= BLK
-    fixed = slots * (ninvp + ninvs) * 8 + 2 * namps * 8 + 2 * slots * ntabs * 8 + 3 * ntabs * 4 + 2 * nflows * 4
+    quad = bool(cfg.get("gather16"))      # 16-byte copies of groups of four table operands instead of one copy per operand
+    nmap = ntabs // 4 if quad else ntabs
+    fixed = slots * (ninvp + ninvs) * 8 + 2 * namps * 8 + 2 * slots * ntabs * 8 + 3 * nmap * 4 + 2 * nflows * 4
     nst_max = max(0, (cfg["smem_kb"] * 1024 - fixed) // (2 * BLK * 8))
     files, binfo = [], []
     exec_hel, exec_slot = 0, 0
@@ -414,7 +418,8 @@ def emit_coop(n, fp32=True, acc_max=24, **over):
         # per member: gather map of the helicity-independent operands, colour-flow map
         bmeta.append((len(flowmap), len(visits)))
         for pi in fam["members"]:
-            visits.append((len(tabmap), b.ntab, len(invmap), b.ninv, len(ampsign), b.plan.namps, len(flowmap), len(b.flows)))
+            assert b.ntab % 4 == 0
+            visits.append((len(tabmap), b.ntab // 4 if quad else b.ntab, len(invmap), b.ninv, len(ampsign), b.plan.namps, len(flowmap), len(b.flows)))
             for nm, off in sorted(b.inv.items(), key=lambda kv: kv[1]):
                 src = inv[_perm_name(nm, pi)]
                 invmap += [src + j for j in range(b.sizes[nm])]
@@ -422,7 +427,9 @@ def emit_coop(n, fp32=True, acc_max=24, **over):
                 o_ = tuple(pi[g] for g in flow_order[f])
                 flowmap.append(2 * flow_index[o_] * BLK)
             m1, isign = _table_maps(b.tables, ftab, pi)
-            tabmap += m1
+            # the relabelling maps whole tabled currents (8 x nv contiguous elements): one map entry per group of four
+            assert all(m1[k] % 4 == 0 and m1[k + 1:k + 4] == [m1[k] + 1, m1[k] + 2, m1[k] + 3] for k in range(0, len(m1), 4))
+            tabmap += m1[0::4] if quad else m1
             ampsign += _amp_signs(b.plan, isign)
         binfo.append(dict(family="%s%d" % (fam["kind"], fam["size"]), members=nm_, terms=len(b.plan.terms), flops=flops,
                           flows=len(touches), staged=len(staged), max_live=b.plan.max_live(), ninv=b.ninv, ntab=b.ntab))
@@ -456,6 +463,10 @@ def _main_unit(E, n, ns, hdr, cfi, cfden, fams, bodies, bmeta, invmap, flowmap, 
                          what="operand maps, table descriptors, invariants kernel, persistent sigma kernel (%d bodies x their "
                               "relabellings, colour sum K6, helicity sum K7), launcher" % nbody)]
     w = out.append
+    quad = bool(cfg.get("gather16"))
+    w("constexpr int NMAP = %d;      // index-map entries per visit: one per table operand, or per group of four (16-byte copies)\n"
+      % (ntabs // 4 if quad else ntabs))
+    w("constexpr bool QUAD = %s;\n" % ("true" if quad else "false"))
     w("constexpr int NINV = %d, NINVP = %d, NINVS = %d, NTABS = %d, NTABF = %d, NST = %d, NBODY = %d, TPOS = %d;\n"
       % (ninv, ninvp, ninvs, ntabs, ntabf, nst, nbody, npar - 3))
 
@@ -580,8 +591,8 @@ def _main_unit(E, n, ns, hdr, cfi, cfden, fams, bodies, bmeta, invmap, flowmap, 
             "    // body %d: family %s%d, %d terms, %d relabellings\n"
             "#pragma unroll 1\n    for (int m = 0; m < %d; ++m) {\n"
             "      const int v = %d + m;\n"
-            "      visit_step<T, SLOTS>(visit_desc, v, tab_map, inv_map, gtab, asgn, flow_map, sinv0, sinvp0, smap0, stab0, ssgn0, sfm0, NINVP, NINVS,\n"
-            "                           NTABS, NTABF, NAMPS, NFLOWS);\n"
+            "      visit_step<T, SLOTS, QUAD>(visit_desc, v, tab_map, inv_map, gtab, asgn, flow_map, sinv0, sinvp0, smap0, stab0, ssgn0, sfm0, NINVP, NINVS,\n"
+            "                                 NTABS, NMAP, NTABF, NAMPS, NFLOWS);\n"
             "      const int hp = permute_helicity<NPAR, NGLU>(h, hel_shift + %d + m * NGLU);\n"
             "      body%d(sinvp, stab0 + (unsigned)(((v & 1) * SLOTS + slot) * NTABS) * SZ, ssgn0 + (unsigned)((v & 1) * NAMPS) * SZ, sj, jamp, hp, live,\n"
             "             sfm0 + (unsigned)((v & 1) * NFLOWS) * 4u);\n    }\n"
@@ -630,8 +641,8 @@ sigma_kernel(long long nevt, int ntb, int tb_first, const T* __restrict__ lane_w
   // shared memory: full per-event operand set | the running visit's helicity-independent operands | amplitude signs [2] |
   // table operands [2] | index maps [3] | staged JAMPs
   const unsigned sinv0 = sbase, sinvp0 = sinv0 + SLOTS * NINVP * SZ, ssgn0 = sinvp0 + SLOTS * NINVS * SZ;
-  const unsigned stab0 = ssgn0 + 2 * NAMPS * SZ, smap0 = stab0 + 2 * SLOTS * NTABS * SZ, sfm0 = smap0 + 3 * NTABS * 4;
-  const unsigned sj = sfm0 + 2 * NFLOWS * 4 + ((NTABS & 1) ? 4 : 0) + tid * SZ;
+  const unsigned stab0 = ssgn0 + 2 * NAMPS * SZ, smap0 = stab0 + 2 * SLOTS * NTABS * SZ, sfm0 = smap0 + 3 * NMAP * 4;
+  const unsigned sj = sfm0 + 2 * NFLOWS * 4 + ((NMAP & 1) ? 4 : 0) + tid * SZ;
   const unsigned sinvp = sinvp0 + slot * NINVS * SZ;
   const T* __restrict__ asgn = amp_sign_of((T*)nullptr);
   constexpr unsigned SINV_BYTES = (SLOTS * NINVP * SZ + 15u) / 16u * 16u;      // the colour sum's tile staging starts behind it
@@ -662,7 +673,7 @@ sigma_kernel(long long nevt, int ntb, int tb_first, const T* __restrict__ lane_w
     const int live = slot_live && wgt != T(0);
     __syncthreads();
     build_tables_global<T>(tab_groups, NGROUPS, tab_desc, sinv0, gtab, NINVP, NTABF, SLOTS, s_tbit);
-    visit_prologue<T, SLOTS>(visit_desc, tab_map, gtab, asgn, flow_map, smap0, stab0, ssgn0, sfm0, NTABS, NTABF, NAMPS, NFLOWS);
+    visit_prologue<T, SLOTS, QUAD>(visit_desc, tab_map, gtab, asgn, flow_map, smap0, stab0, ssgn0, sfm0, NTABS, NMAP, NTABF, NAMPS, NFLOWS);
 %(calls)s
     visit_drain();
     // nothing reads the invariant block after the last visit: the next group's invariants travel during the colour sum
@@ -696,7 +707,7 @@ static int run(const double* mom, T* me_out, long long nevt, const T* lane_w, in
   norm /= (double)%(cfden)d * (double)%(denom)d;
   int dev = 0, nsm = 0, per_sm = 0;
   if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return -1;
-  size_t smem = (size_t)(SLOTS * (NINVP + NINVS) + 2 * NAMPS + 2 * SLOTS * NTABS + 2 * NST * BLK) * sizeof(T) + 3 * NTABS * 4 + 2 * NFLOWS * 4 + 8;
+  size_t smem = (size_t)(SLOTS * (NINVP + NINVS) + 2 * NAMPS + 2 * SLOTS * NTABS + 2 * NST * BLK) * sizeof(T) + 3 * NMAP * 4 + 2 * NFLOWS * 4 + 8;
   if (sizeof(T) == 8 && smem < COLOUR_SMEM) smem = COLOUR_SMEM;
   auto kern = sigma_kernel<T>;
   if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return -1;
