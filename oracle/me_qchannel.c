@@ -28,9 +28,8 @@
  * Pins (tests/test_oracle_qchannel.py): the textbook closed form of q q~ -> t t~ (absolute normalisation, colour
  * average), the Ward identity on every gluon of every process (relative signs between diagram classes), the
  * initial-state collinear limits q -> q g and g -> q q~ onto the closed form (every 1-jet process) and of
- * q q~ -> t t~ g g onto q q~ -> t t~ g, C- and beam-exchange symmetries.  The other 2-jet crossings with one light line
- * (q g -> t t~ q g, g g -> t t~ q q~, ...) run the same code with other external spinors; their own pins are the Ward
- * identities.  Two light lines: see the test file's header; the SIGN of the interference between the two pairings of the
+ * q q~ -> t t~ g g, q g -> t t~ q g and g g -> t t~ q q~ onto the 1-jet processes, C- and beam-exchange symmetries for
+ * the mirrored crossings.  Two light lines: see the test file's header; the SIGN of the interference between the two pairings of the
  * same-flavour processes is a reading with no pin of its own ("parity unpinned" for that term).
  */
 #include "oracle_internal.h"

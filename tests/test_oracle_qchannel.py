@@ -10,7 +10,8 @@ None of these re-types the oracle's recursion:
         q -> q g :  |M|^2 -> g^2 C_F (1 + x^2)/(1 - x) / (x p_a.k) |M_0(x p_a)|^2
         g -> q q~:  |M|^2 -> g^2 T_R (x^2 + (1 - x)^2) / (x p_a.k) |M_0(x p_a)|^2
     — fixes the normalisation of every 1-jet process (incoming-gluon colour and spin averages included), and of the
-    2-jet process q q~ -> t t~ g g against the 1-jet one;
+    2-jet processes q q~ -> t t~ g g, q g -> t t~ q g and g g -> t t~ q q~ against the 1-jet ones (their beam and C mirrors
+    against them);
   * charge conjugation (q <-> q~ together with t <-> t~) and beam exchange;
   * two light-quark lines (flavours q and r): the final-state collinear limit r r~ -> g of q q~ -> t t~ r r~ onto
     q q~ -> t t~ g with <P_qg> = T_R (1 - 2 z (1 - z)) (two azimuths pi/2 apart cancel the spin correlation), the
@@ -149,6 +150,35 @@ def test_charge_conjugation_and_beam_exchange(orc):
         assert abs(orc.me_qchannel("qgtTq", p) / orc.me_qchannel("QgtTQ", c) - 1) < 1e-10
         b = p[[1, 0, 2, 3, 4]]                   # beams exchanged
         assert abs(orc.me_qchannel("qgtTq", p) / orc.me_qchannel("gqtTq", b) - 1) < 1e-10
+
+
+def test_other_two_jet_crossings_collinear_limits_and_mirrors(orc):
+    """The 2-jet crossings with one light line that the test above does not reach: q g -> t t~ q g with the final gluon
+    along the incoming quark (q -> q g onto q g -> t t~ q) and g g -> t t~ q q~ with the final antiquark along an incoming
+    gluon (g -> q q~ onto q g -> t t~ q); then the beam- and C-mirrored processes against these two."""
+    x, theta = 0.7, 1e-3
+    hard = np.array([0.0, 60.0, -80.0, 66.0])
+    hard[0] = np.linalg.norm(hard[1:])
+    pa, pb, t, tb, k = _collinear_event(x, theta, 0, extra=hard)
+    p6 = np.array([pa, pb, t, tb, hard, k])
+    ref = np.array([x * pa, pb, t, tb, hard])
+    jobs = {
+        "qgtTqg": ("qgtTqg", p6), "ggtTqQ": ("ggtTqQ", p6), "ref": ("qgtTq", ref),
+        "gqtTqg": ("gqtTqg", p6[[1, 0, 2, 3, 4, 5]]),                 # beams exchanged
+        "QgtTQg": ("QgtTQg", p6[[0, 1, 3, 2, 4, 5]]),                 # charge conjugation: q <-> q~, t <-> t~
+        "gQtTQg": ("gQtTQg", p6[[1, 0, 3, 2, 4, 5]]),
+        "QqtTgg": ("QqtTgg", p6[[1, 0, 2, 3, 4, 5]]), "qQtTgg": ("qQtTgg", p6),
+    }
+    with ThreadPoolExecutor(8) as ex:
+        val = dict(zip(jobs, ex.map(lambda kv: orc.me_qchannel(*kv), jobs.values())))
+    pk = mdot(pa, k)
+    r1 = val["qgtTqg"] / (G2 * CF * (1 + x * x) / (1 - x) / (x * pk) * val["ref"])
+    r2 = val["ggtTqQ"] / (G2 * TR * (x * x + (1 - x) ** 2) / (x * pk) * val["ref"])
+    assert abs(r1 - 1) < 3e-3 and abs(r2 - 1) < 3e-3, (r1, r2)
+    assert abs(val["gqtTqg"] / val["qgtTqg"] - 1) < 1e-10
+    assert abs(val["QgtTQg"] / val["qgtTqg"] - 1) < 1e-10
+    assert abs(val["gQtTQg"] / val["qgtTqg"] - 1) < 1e-10
+    assert abs(val["QqtTgg"] / val["qQtTgg"] - 1) < 1e-10
 
 
 def _perp(k):
