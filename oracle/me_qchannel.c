@@ -269,7 +269,9 @@ static void amplitude(const qspec* s, const qtab* t, const qext* x, int pairing,
   }
 }
 
-double oracle_me_qchannel(const char* spec, const double* p, const oracle_params_t* par, double* hel_out, int ward_which) {
+/* pauli != 0: only the helicity and colour configurations in which the two identical final-state quarks (particles 4 and 5)
+ * are in the same spin and colour state are summed (diagnostic for the Pauli-principle pin) */
+static double me_q(const char* spec, const double* p, const oracle_params_t* par, double* hel_out, int ward_which, int pauli) {
   qspec s;
   if (parse_spec(spec, &s) != 0) return -1;
   const int npar = s.npar, ng = s.ng, nhel = 1 << npar;
@@ -283,6 +285,7 @@ double oracle_me_qchannel(const char* spec, const double* p, const oracle_params
   real total = 0;
   for (int h = 0; h < nhel; ++h) {
     #define LAM(i) (((h >> (npar - 1 - (i))) & 1) ? 1 : -1)
+    if (pauli && LAM(4) != LAM(5)) { if (hel_out) hel_out[h] = 0; continue; }
     qext x;
     for (int g = 0; g < ng; ++g) {
       int ip = s.gpart[g];
@@ -310,6 +313,7 @@ double oracle_me_qchannel(const char* spec, const double* p, const oracle_params
       int gcol[3] = {0, 0, 0}; { int64_t r = ic; for (int g = 0; g < ng; ++g) { gcol[g] = (int)(r % 8); r /= 8; } }
       for (int iq = 0; iq < nqcol; ++iq) {
         int qcolour[8] = {0, 0, 0, 0, 0, 0, 0, 0}; { int r = iq; for (int k = 0; k < nq; ++k) { qcolour[qpart[k]] = r % 3; r /= 3; } }
+        if (pauli && qcolour[4] != qcolour[5]) continue;
         cplx M[3][3]; memset(M, 0, sizeof(M));
         for (int k = 0; k < s.npairing; ++k) {
           cplx Mk[3][3];
@@ -325,6 +329,18 @@ double oracle_me_qchannel(const char* spec, const double* p, const oracle_params
   }
   free(t);
   return (double)(total / s.denom);
+}
+
+double oracle_me_qchannel(const char* spec, const double* p, const oracle_params_t* par, double* hel_out, int ward_which) {
+  return me_q(spec, p, par, hel_out, ward_which, 0);
+}
+/* Pauli principle (pin of the relative sign of the two pairings): for two identical final-state quarks with the same
+ * momentum, helicity and colour the amplitude vanishes.  Returns the part of |M|^2 (same normalisation) from the
+ * configurations with equal helicity and colour of particles 4 and 5; the caller passes p4 = p5.  -1 unless the
+ * process ends in two identical (anti)quarks. */
+double oracle_me_qchannel_pauli(const char* spec, const double* p, const oracle_params_t* par) {
+  if (strlen(spec) != 6 || spec[4] != spec[5] || (spec[4] != 'q' && spec[4] != 'Q')) return -1;
+  return me_q(spec, p, par, NULL, -1, 1);
 }
 
 int oracle_me_qchannel_batch(const char* spec, const double* momenta, int64_t nevt, const oracle_params_t* par,

@@ -93,6 +93,7 @@ double oracle_me_ggttng_ward(int nfinal_gluons, const double* p, const oracle_pa
  * Colour-dressed Feynman rules with explicit colour sums (me_qchannel.c).  ward_which >= 0: gluon number ward_which
  * (in process order among the gluons) has its polarisation replaced by its momentum; -1: physical. ---- */
 double oracle_me_qchannel(const char* spec, const double* p, const oracle_params_t* par, double* hel_out, int ward_which);
+double oracle_me_qchannel_pauli(const char* spec, const double* p, const oracle_params_t* par);   /* see me_qchannel.c */
 int oracle_me_qchannel_batch(const char* spec, const double* momenta, int64_t nevt, const oracle_params_t* par,
                              double* me_out, int nthreads);
 

@@ -58,6 +58,8 @@ class Oracle:
         L.oracle_me_batch.argtypes = [C.c_int, _dp, C.c_int64, C.POINTER(Params), _dp, C.c_int]
         L.oracle_me_qchannel.restype = C.c_double
         L.oracle_me_qchannel.argtypes = [C.c_char_p, _dp, C.POINTER(Params), _dp, C.c_int]
+        L.oracle_me_qchannel_pauli.restype = C.c_double
+        L.oracle_me_qchannel_pauli.argtypes = [C.c_char_p, _dp, C.POINTER(Params)]
         L.oracle_me_qchannel_batch.argtypes = [C.c_char_p, _dp, C.c_int64, C.POINTER(Params), _dp, C.c_int]
         L.oracle_weight_max.argtypes = [_dp, _dp, C.c_int64, C.c_int, _dp, _dp]
 
@@ -142,6 +144,11 @@ class Oracle:
         hel = np.zeros(1 << len(spec)) if per_helicity else None
         v = self.lib.oracle_me_qchannel(spec.encode(), _p(p), C.byref(par), _p(hel) if per_helicity else None, C.c_int(ward))
         return (v, hel) if per_helicity else v
+
+    def me_qchannel_pauli(self, spec, p, par=None):
+        """Part of |M|^2 from equal helicity and colour of the two identical final quarks (oracle.h)."""
+        par = par or default_params(); p = np.ascontiguousarray(p, dtype=np.float64)
+        return self.lib.oracle_me_qchannel_pauli(spec.encode(), _p(p), C.byref(par))
 
     def me_qchannel_batch(self, spec, momenta, par=None, nthreads=0):
         par = par or default_params()
