@@ -35,8 +35,9 @@ BLK = 256      # default threads per CTA (cfg["block"])
 # (measured on B200: gg -> tt~gg 37.9 ms with (2, 1) tables and 40-term bodies against 40.6 ms with (3, 2)
 # and 24; gg -> tt~ggg with (3, 2) and 16-term bodies: 424 ms against 500 / 562 ms with 32 / 48 at that stage; l2_window: the
 # scratch as a persisting L2 window, 387 -> 373 ms; gather16: 16-byte copies of groups of four table operands, 366 -> 355 ms,
-# but 37.7 -> 38.3 ms at n = 4)
-TUNED = {4: dict(max_phase=40, gtab=2, qtab=1, smem_kb=110, block=128, sync_every=0),
+# but 37.7 -> 38.3 ms at n = 4; merge_complement: classes over k- and (n - k)-subsets share bodies, 15 -> 11 visits at n = 4,
+# 37.7 -> 36.6 ms (fp32 24.9 -> 22.6), no change at n = 5 (135 -> 115 visits, 355 -> 356 ms))
+TUNED = {4: dict(max_phase=40, gtab=2, qtab=1, smem_kb=110, block=128, sync_every=0, merge_complement=True),
          5: dict(max_phase=16, gtab=3, qtab=2, smem_kb=110, block=128, sync_every=0, min_class=5, l2_window=True, gather16=True)}
 INV_SIZE = {"sg": 1, "pm": 4, "tl": 5, "tr": 5, "eg": 5, "ub": 16, "vv": 16}
 _ORDER = {"s": 0, "p": 1, "t": 2, "e": 3, "u": 4, "v": 5}
@@ -84,12 +85,14 @@ def _pack(groups, limit):
     return [b for b in bodies if b]
 
 
-def families(n, max_phase, min_class=6):
+def families(n, max_phase, min_class=6, merge_complement=False):
     """[dict(kind, size, members=[pi, ...], bodies=[[term, ...], ...])]: the canonical class of every family, cut into
     bodies, and the relabellings pi (tuples: canonical gluon i -> actual gluon pi[i]) of its members.  Classes with
     fewer than `min_class` terms are not worth a visit per member: small classes over the same gluon subsets (same
     relabellings) are merged into one family if that makes them big enough, the rest is emitted as it is, together, in a
-    last family with the identity as its only member."""
+    last family with the identity as its only member.  merge_complement: classes over k-subsets and over (n - k)-subsets
+    (k != n - k) become one family too — keyed by the complement, the smaller classes have the same relabellings — so
+    that their terms share bodies (fewer visits per event group)."""
     classes = {}
     for term in topo.diagram_terms(n):
         kind, S = family_key(term, n)
@@ -114,6 +117,17 @@ def families(n, max_phase, min_class=6):
             normal.append(("+".join(k for k, _ in lst), size, merged))
         else:
             misc += [t for _, cls in lst for S in sorted(cls) for t in cls[S]]
+    if merge_complement:
+        byk = {}
+        for kind, size, cls in normal:
+            big = max(size, n - size)
+            if size != big:                   # re-key by the complement: same subsets as the (n - size)-classes
+                cls = {tuple(i for i in range(n) if i not in S): ts for S, ts in cls.items()}
+            grp = byk.setdefault(big, dict(kinds=[], cls={}))
+            grp["kinds"].append(kind + ("c" if size != big else ""))
+            for S, ts in cls.items():
+                grp["cls"].setdefault(S, []).extend(ts)
+        normal = [("+".join(g["kinds"]), big, g["cls"]) for big, g in sorted(byk.items())]
     for kind, size, cls in normal:
         S0 = min(cls)
         rest0 = [i for i in range(n) if i not in S0]
@@ -309,7 +323,7 @@ def emit_coop(n, fp32=True, acc_max=24, **over):
     cfi = [[int(v * cfden) for v in row] for row in cf]
     flow_index = topo.flow_index_table(n)
     flow_order = {i: p for p, i in flow_index.items()}
-    fams = families(n, cfg["max_phase"], cfg.get("min_class", 6))
+    fams = families(n, cfg["max_phase"], cfg.get("min_class", 6), cfg.get("merge_complement", False))
     # bodies are compiled for the register budget of the kernel's occupancy target (build.py reads the "nvcc:" line)
     maxreg = min(255, 65536 // (BLK * cfg.get("ctas_per_sm", 256 // BLK)) // 8 * 8)
     hdr = dict(proc=proc, n=n, ncol=ncol, nhel=nhel, ns=ns, npar=npar, nlane=nlane, blk=BLK,
